@@ -1,0 +1,10 @@
+"""CPU oracle for the mphv hot path -- TEST INFRASTRUCTURE, not the product.
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package. It shares no code with
+``paper_2305_01487_b200`` (the CUDA path) and neither imports the other.
+"""
+from .binding import (  # noqa: F401
+    Grid, Box, build, lib, sweep_pencil, sweep_x, sweep_v, step, moments, total, num_threads,
+    BC_PERIODIC, BC_OUTFLOW, BC_WALL, OK, ERR_ARG, ERR_RANGE,
+)

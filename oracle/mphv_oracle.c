@@ -1,0 +1,399 @@
+/*
+ * mphv_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, step-by-step CPU statement (fp64, no FMA contraction: build with
+ * -ffp-contract=off) of the kinetic Vlasov hot path of muphyII (arXiv 2305.01487):
+ * dimensionally split 1-D conservative, positivity-preserving, third-order
+ * semi-Lagrangian (PFC) sweeps of f(x,v) plus the velocity moments n, j, P.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl
+ * reference legs may call this. It shares no code, header, table or helper with
+ * the CUDA path under paper_2305_01487_b200/csrc and neither includes the other.
+ *
+ * What the paper fixes (PAPER.md = /root/reference/PAPER.md, cited "P:Lnnn"):
+ *   - eq. (1), P:L53 (sec. 2): df/dt + v.grad_x f + (q/m)(E + v x B).grad_v f = 0
+ *   - P:L135 (sec. 4.1): "semi-Lagrangian scheme using the positive and
+ *     flux-conservative (PFC) method", "spatially third-order version", "limiter
+ *     only for small values of the phase space distribution function to guarantee
+ *     positivity", Strang splitting x<->v, further splitting into the three
+ *     spatial and three velocity directions.
+ *   - P:L57 (sec. 2): n = int f dv, n u = int v f dv, P = m int v v f dv.
+ *   - P:L187 (sec. 4.3): two boundary cells.
+ * The paper prints no flux/limiter formula; the formulas below are the readings
+ * listed in DESIGN.md ("Readings of the paper", R1..R14) = SURVEY.md sec. 8(c).
+ *
+ * Pins (tests/test_oracle_pins.py, all -m "not gpu"): integer-Courant exact
+ * translation, exact-rational remap brute force, quadratic exactness, mass
+ * conservation, positivity, mirror symmetry, free streaming, gyration closure,
+ * uniform-E shift, Maxwellian and hand-summed moments.
+ * PARITY UNPINNED against the authors' own implementation: PAPER.md prints no
+ * value of their scheme's output anywhere.
+ *
+ * Layouts (C order, fastest index last, interior cells only, no stored halo):
+ *   f    [nz][ny][nx][nvz][nvy][nvx]
+ *   E, B [3][nz][ny][nx]            (component-major, cell-centred, reading R8)
+ *   n    [nz][ny][nx];  j [3][nz][ny][nx];  P [6][nz][ny][nx] (xx,xy,xz,yy,yz,zz)
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef struct {
+    int32_t nx[3];   /* spatial extents x,y,z; 1 = inactive                     */
+    int32_t nv[3];   /* velocity extents vx,vy,vz; 1 = inactive (v == 0, dv == 1) */
+    int32_t bc[3];   /* per spatial dim: 0 periodic, 1 outflow (zero gradient)  */
+} orc_grid;
+
+typedef struct {
+    double xlo[3], xhi[3], vlo[3], vhi[3];   /* cells tile [lo,hi) */
+} orc_box;
+
+enum { ORC_BC_PERIODIC = 0, ORC_BC_OUTFLOW = 1, ORC_BC_WALL = 2 };
+enum { ORC_OK = 0, ORC_ERR_ARG = 1, ORC_ERR_RANGE = 3 };
+
+/* ---- c-1 grid: cell-centred finite volumes (reading R1) --------------------- */
+static double cell_width(double lo, double hi, int n) { return (hi - lo) / (double)n; }
+
+/* centre of velocity cell j along dim d; inactive dimension => 0 (sec. 8b) */
+static double v_centre(const orc_grid *g, const orc_box *b, int d, int j)
+{
+    if (g->nv[d] == 1) return 0.0;
+    double dv = cell_width(b->vlo[d], b->vhi[d], g->nv[d]);
+    return b->vlo[d] + ((double)j + 0.5) * dv;
+}
+static double v_width(const orc_grid *g, const orc_box *b, int d)
+{
+    if (g->nv[d] == 1) return 1.0;
+    return cell_width(b->vlo[d], b->vhi[d], g->nv[d]);
+}
+
+/* ---- c-6 boundary rule for reading a pencil value at any index -------------- */
+static double fetch(const double *f, int n, long idx, int bc)
+{
+    if (idx >= 0 && idx < n) return f[idx];
+    if (bc == ORC_BC_PERIODIC) {
+        long m = idx % n;
+        if (m < 0) m += n;
+        return f[m];
+    }
+    if (bc == ORC_BC_OUTFLOW) return idx < 0 ? f[0] : f[n - 1];   /* zero gradient */
+    return 0.0;                                                   /* velocity wall: empty ghosts */
+}
+
+/* ---- c-4 limited slopes: PFC positivity correctors, division-free ----------
+ * eps+ = min(1, 2 g_i / d+) for d+ > 0 else 1;  L+ = eps+ d+
+ * eps- = min(1, -2 g_i / d-) for d- < 0 else 1; L- = eps- d-
+ * (the upper-bound correctors of the full PFC method are dropped: "limiter only
+ *  for small values ... to guarantee positivity", reading R2)          */
+static double slope_plus(double gi, double gip1)
+{
+    double dp = gip1 - gi;
+    if (dp > 0.0) { double cap = 2.0 * gi; return dp < cap ? dp : cap; }
+    return dp;
+}
+static double slope_minus(double gim1, double gi)
+{
+    double dm = gi - gim1;
+    if (dm < 0.0) { double cap = -2.0 * gi; return dm > cap ? dm : cap; }
+    return dm;
+}
+
+/*
+ * One 1-D PFC-3 remap of a pencil of n cell averages by Courant number s
+ * (displacement in cells, towards +index for s > 0). in and out must not alias.
+ * phi_lo / phi_hi (optional) receive the flux through faces -1/2 and n-1/2 in
+ * units of (cell width x f): mass leaving through the high face is +phi_hi,
+ * mass entering through the low face is +phi_lo.
+ * P:L135; readings R1-R3, R6, R7, R11, R12.
+ */
+int orc_sweep_pencil(const double *in, double *out, int n, double s, int bc,
+                     double *phi_lo, double *phi_hi)
+{
+    if (!in || !out || n < 1 || !(s == s) || isinf(s)) return ORC_ERR_ARG;
+    if (bc != ORC_BC_PERIODIC && !(fabs(s) < 1.0)) return ORC_ERR_RANGE;
+
+    /* c-3 shift split, sign-symmetric (reading R11) */
+    long k;
+    double frac;                        /* alpha for s >= 0, beta for s < 0 */
+    if (s >= 0.0) { double fl = floor(s); k = (long)fl; frac = s - fl; }
+    else          { double ce = ceil(s);  k = (long)ce; frac = ce - s; }
+
+    /* g_i = f_{i-k} through the boundary rule, for i = -2 .. n+1 */
+    double *g = (double *)malloc((size_t)(n + 4) * sizeof(double));
+    double *phi = (double *)malloc((size_t)(n + 1) * sizeof(double));  /* phi[i+1] = phi_{i+1/2}, i=-1..n-1 */
+    if (!g || !phi) { free(g); free(phi); return ORC_ERR_ARG; }
+    for (long i = -2; i < n + 2; ++i) g[i + 2] = fetch(in, n, i - k, bc);
+#define G(i) g[(i) + 2]
+
+    /* c-5 fractional flux at every face i+1/2, i = -1 .. n-1 */
+    double c1 = ((1.0 - frac) * (2.0 - frac)) / 6.0;
+    double c2 = ((1.0 - frac) * (1.0 + frac)) / 6.0;
+    for (long i = -1; i < n; ++i) {
+        double ph;
+        if (s >= 0.0) {
+            double Lp = slope_plus(G(i), G(i + 1));
+            double Lm = slope_minus(G(i - 1), G(i));
+            ph = frac * ((G(i) + c1 * Lp) + c2 * Lm);
+        } else {
+            double Lm = slope_minus(G(i), G(i + 1));
+            double Lp = slope_plus(G(i + 1), G(i + 2));
+            ph = -frac * ((G(i + 1) - c1 * Lm) - c2 * Lp);
+        }
+        phi[i + 1] = ph;
+    }
+    /* c-6: closed velocity box: no flux through the two wall faces (reading R7) */
+    if (bc == ORC_BC_WALL) { phi[0] = 0.0; phi[n] = 0.0; }
+
+    /* update: difference of fluxes first, then added to g */
+    for (long i = 0; i < n; ++i) out[i] = G(i) + (phi[i] - phi[i + 1]);
+#undef G
+    if (phi_lo) *phi_lo = phi[0];
+    if (phi_hi) *phi_hi = phi[n];
+    free(g); free(phi);
+    return ORC_OK;
+}
+
+/* ---- index helpers for the 6-D array ---------------------------------------- */
+static size_t n_space(const orc_grid *g) { return (size_t)g->nx[0] * g->nx[1] * g->nx[2]; }
+static size_t n_vel(const orc_grid *g)   { return (size_t)g->nv[0] * g->nv[1] * g->nv[2]; }
+
+static int grid_ok(const orc_grid *g, const orc_box *b)
+{
+    if (!g || !b) return 0;
+    for (int d = 0; d < 3; ++d) {
+        if (g->nx[d] < 1 || g->nv[d] < 1) return 0;
+        if (g->bc[d] != ORC_BC_PERIODIC && g->bc[d] != ORC_BC_OUTFLOW) return 0;
+        if (g->nx[d] > 1 && !(b->xhi[d] > b->xlo[d])) return 0;
+        if (g->nv[d] > 1 && !(b->vhi[d] > b->vlo[d])) return 0;
+    }
+    return 1;
+}
+
+size_t orc_f_count(const orc_grid *g) { return g ? n_space(g) * n_vel(g) : 0; }
+
+/*
+ * Spatial sweep S_d(dt): every pencil along spatial dim d is remapped with
+ * s = v_d dt / dx_d, v_d the cell-centre velocity (c-2; eq. (1) term v.grad_x f,
+ * P:L53). net_out (optional) accumulates sum over pencils of (phi_hi - phi_lo),
+ * i.e. the mass (in units of cell-volume x f) that left through the two ends of
+ * the axis (zero on a periodic axis).
+ */
+int orc_sweep_x(double *f, const orc_grid *g, const orc_box *b, int dim, double dt,
+                double *net_out)
+{
+    if (!f || !grid_ok(g, b) || dim < 0 || dim > 2 || g->nx[dim] < 2) return ORC_ERR_ARG;
+    if (!(dt == dt) || isinf(dt)) return ORC_ERR_ARG;
+    const int n = g->nx[dim];
+    const double dx = cell_width(b->xlo[dim], b->xhi[dim], n);
+    const size_t nvel = n_vel(g);
+    /* strides in doubles */
+    size_t sstride[3];
+    sstride[0] = nvel;
+    sstride[1] = (size_t)g->nx[0] * nvel;
+    sstride[2] = (size_t)g->nx[1] * g->nx[0] * nvel;
+    const size_t stride = sstride[dim];
+    const int bc = g->bc[dim];
+
+    /* range check first: a failed call leaves f untouched */
+    if (bc != ORC_BC_PERIODIC)
+        for (int j = 0; j < g->nv[dim]; ++j) {
+            double s = (v_centre(g, b, dim, j) * dt) / dx;
+            if (!(fabs(s) < 1.0)) return ORC_ERR_RANGE;
+        }
+
+    /* the other two spatial dims */
+    const int da = (dim + 1) % 3, db = (dim + 2) % 3;
+    long double net = 0.0L;
+    int status = ORC_OK;
+#pragma omp parallel
+    {
+        double *pin = (double *)malloc((size_t)n * sizeof(double));
+        double *pout = (double *)malloc((size_t)n * sizeof(double));
+        long double my_net = 0.0L;
+#pragma omp for collapse(2) schedule(static)
+        for (int ia = 0; ia < g->nx[da]; ++ia)
+            for (int ib = 0; ib < g->nx[db]; ++ib) {
+                size_t base_s = (size_t)ia * sstride[da] + (size_t)ib * sstride[db];
+                for (int jz = 0; jz < g->nv[2]; ++jz)
+                    for (int jy = 0; jy < g->nv[1]; ++jy)
+                        for (int jx = 0; jx < g->nv[0]; ++jx) {
+                            int jv[3] = { jx, jy, jz };
+                            double s = (v_centre(g, b, dim, jv[dim]) * dt) / dx;
+                            size_t base = base_s + ((size_t)jz * g->nv[1] + jy) * g->nv[0] + jx;
+                            for (int i = 0; i < n; ++i) pin[i] = f[base + (size_t)i * stride];
+                            double plo, phi;
+                            int st = orc_sweep_pencil(pin, pout, n, s, bc, &plo, &phi);
+                            if (st != ORC_OK) {
+#pragma omp critical
+                                status = st;
+                                continue;
+                            }
+                            for (int i = 0; i < n; ++i) f[base + (size_t)i * stride] = pout[i];
+                            my_net += (long double)phi - (long double)plo;
+                        }
+            }
+#pragma omp critical
+        net += my_net;
+        free(pin); free(pout);
+    }
+    if (net_out) *net_out = (double)net;
+    return status;
+}
+
+/* c-2 Lorentz acceleration component d at one spatial cell, plain fp64,
+ * left-to-right, no FMA: a_d = (q/m)(E_d + (v x B)_d); eq. (1). */
+static double accel(int d, double qm, const double E[3], const double B[3], const double v[3])
+{
+    double cross;
+    if (d == 0)      cross = v[1] * B[2] - v[2] * B[1];
+    else if (d == 1) cross = v[2] * B[0] - v[0] * B[2];
+    else             cross = v[0] * B[1] - v[1] * B[0];
+    return qm * (E[d] + cross);
+}
+
+/*
+ * Velocity sweep V_d(dt): every pencil along velocity dim d is remapped with
+ * s = a_d dt / dv_d (constant along the pencil because (v x B)_d does not
+ * contain v_d). Velocity box is closed: empty ghosts, zero wall flux (R7).
+ * E, B: [3][nz][ny][nx] cell-centred.
+ */
+int orc_sweep_v(double *f, const orc_grid *g, const orc_box *b, double q_over_m,
+                const double *E, const double *B, int dim, double dt)
+{
+    if (!f || !E || !B || !grid_ok(g, b) || dim < 0 || dim > 2 || g->nv[dim] < 2) return ORC_ERR_ARG;
+    if (!(dt == dt) || isinf(dt)) return ORC_ERR_ARG;
+    const int n = g->nv[dim];
+    const double dv = v_width(g, b, dim);
+    const size_t ns = n_space(g), nvel = n_vel(g);
+    size_t vstride[3] = { 1, (size_t)g->nv[0], (size_t)g->nv[0] * g->nv[1] };
+    const size_t stride = vstride[dim];
+    const int da = (dim + 1) % 3, db = (dim + 2) % 3;
+
+    /* range check first (closed box needs |s| < 1): a failed call leaves f untouched */
+    for (size_t c = 0; c < ns; ++c) {
+        double Ec[3] = { E[c], E[ns + c], E[2 * ns + c] };
+        double Bc[3] = { B[c], B[ns + c], B[2 * ns + c] };
+        for (int ja = 0; ja < g->nv[da]; ++ja)
+            for (int jb = 0; jb < g->nv[db]; ++jb) {
+                double v[3];
+                v[dim] = 0.0; v[da] = v_centre(g, b, da, ja); v[db] = v_centre(g, b, db, jb);
+                double s = (accel(dim, q_over_m, Ec, Bc, v) * dt) / dv;
+                if (!(fabs(s) < 1.0)) return ORC_ERR_RANGE;
+            }
+    }
+
+    int status = ORC_OK;
+#pragma omp parallel
+    {
+        double *pin = (double *)malloc((size_t)n * sizeof(double));
+        double *pout = (double *)malloc((size_t)n * sizeof(double));
+#pragma omp for schedule(static)
+        for (long long cc = 0; cc < (long long)ns; ++cc) {
+            size_t c = (size_t)cc;
+            double Ec[3] = { E[c], E[ns + c], E[2 * ns + c] };
+            double Bc[3] = { B[c], B[ns + c], B[2 * ns + c] };
+            double *cube = f + c * nvel;
+            for (int ja = 0; ja < g->nv[da]; ++ja)
+                for (int jb = 0; jb < g->nv[db]; ++jb) {
+                    double v[3];
+                    v[dim] = 0.0; v[da] = v_centre(g, b, da, ja); v[db] = v_centre(g, b, db, jb);
+                    double s = (accel(dim, q_over_m, Ec, Bc, v) * dt) / dv;
+                    size_t base = (size_t)ja * vstride[da] + (size_t)jb * vstride[db];
+                    for (int i = 0; i < n; ++i) pin[i] = cube[base + (size_t)i * stride];
+                    int st = orc_sweep_pencil(pin, pout, n, s, ORC_BC_WALL, NULL, NULL);
+                    if (st != ORC_OK) {
+#pragma omp critical
+                        status = st;
+                        continue;
+                    }
+                    for (int i = 0; i < n; ++i) cube[base + (size_t)i * stride] = pout[i];
+                }
+        }
+        free(pin); free(pout);
+    }
+    return status;
+}
+
+/*
+ * c-7 full split step: S_x, S_y, S_z then V_vx, V_vy, V_vz, each with the full
+ * dt, inactive dimensions skipped, fields frozen (readings R4, R5).
+ * net_out (optional): summed outflow of the spatial sweeps, as in orc_sweep_x.
+ */
+int orc_step(double *f, const orc_grid *g, const orc_box *b, double q_over_m,
+             const double *E, const double *B, double dt, double *net_out)
+{
+    if (!grid_ok(g, b)) return ORC_ERR_ARG;
+    double net = 0.0;
+    for (int d = 0; d < 3; ++d)
+        if (g->nx[d] > 1) {
+            double part = 0.0;
+            int st = orc_sweep_x(f, g, b, d, dt, &part);
+            if (st != ORC_OK) return st;
+            net += part;
+        }
+    for (int d = 0; d < 3; ++d)
+        if (g->nv[d] > 1) {
+            int st = orc_sweep_v(f, g, b, q_over_m, E, B, d, dt);
+            if (st != ORC_OK) return st;
+        }
+    if (net_out) *net_out = net;
+    return ORC_OK;
+}
+
+/*
+ * c-8 moments by the midpoint rule at velocity cell centres (readings R9,
+ * R10): n = sum f dV, j_a = sum v_a f dV, P_ab = sum v_a v_b f dV (no q, no m),
+ * dV = dvx dvy dvz, summed in long double so this is the more accurate side.
+ */
+int orc_moments(const double *f, const orc_grid *g, const orc_box *b,
+                double *n_out, double *j_out, double *P_out)
+{
+    if (!f || !n_out || !j_out || !P_out || !grid_ok(g, b)) return ORC_ERR_ARG;
+    const size_t ns = n_space(g), nvel = n_vel(g);
+    const long double dV = (long double)v_width(g, b, 0) * v_width(g, b, 1) * v_width(g, b, 2);
+#pragma omp parallel for schedule(static)
+    for (long long cc = 0; cc < (long long)ns; ++cc) {
+        size_t c = (size_t)cc;
+        const double *cube = f + c * nvel;
+        long double m0 = 0, m1[3] = { 0, 0, 0 }, m2[6] = { 0, 0, 0, 0, 0, 0 };
+        for (int jz = 0; jz < g->nv[2]; ++jz)
+            for (int jy = 0; jy < g->nv[1]; ++jy)
+                for (int jx = 0; jx < g->nv[0]; ++jx) {
+                    long double fv = cube[((size_t)jz * g->nv[1] + jy) * g->nv[0] + jx];
+                    long double vx = v_centre(g, b, 0, jx), vy = v_centre(g, b, 1, jy), vz = v_centre(g, b, 2, jz);
+                    m0 += fv;
+                    m1[0] += vx * fv; m1[1] += vy * fv; m1[2] += vz * fv;
+                    m2[0] += vx * vx * fv; m2[1] += vx * vy * fv; m2[2] += vx * vz * fv;
+                    m2[3] += vy * vy * fv; m2[4] += vy * vz * fv; m2[5] += vz * vz * fv;
+                }
+        n_out[c] = (double)(m0 * dV);
+        for (int a = 0; a < 3; ++a) j_out[(size_t)a * ns + c] = (double)(m1[a] * dV);
+        for (int a = 0; a < 6; ++a) P_out[(size_t)a * ns + c] = (double)(m2[a] * dV);
+    }
+    return ORC_OK;
+}
+
+/* Sum of all entries of f in long double (mass in units of cell volume). */
+double orc_sum(const double *f, size_t count)
+{
+    long double acc = 0.0L;
+    for (size_t i = 0; i < count; ++i) acc += (long double)f[i];
+    return (double)acc;
+}
+
+int orc_num_threads(void)
+{
+    int nt = 1;
+#ifdef _OPENMP
+#pragma omp parallel
+    {
+#pragma omp single
+        nt = omp_get_num_threads();
+    }
+#endif
+    return nt;
+}
