@@ -1,0 +1,327 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the mphv hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl mphv|reference]
+
+A step = one pass of the whole hot path over the workload: the full split step S_x, S_y, [S_z],
+V_vx, V_vy, V_vz followed by the moments n, j, P (mphv_step_moments through the C ABI).
+Metric: phase-space cell-updates/s = cells x steps / time (BASELINE.json), fp64.
+N = 1 runs BASELINE.json configs[3] (2D3V 128x64x40^3, the headline roofline config).
+N > 1 (torchrun): every rank advances its own seeded copy of that workload (independent
+problems, no data-path collective), scaling = weak; time = max over ranks.
+--impl reference times the CPU oracle (oracle/) on a bounded spatial sub-block of the same
+workload on the host cores; rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+from pathlib import Path
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+import numpy as np
+
+METRIC = "phase_space_cell_updates_per_sec"
+UNIT = "cell-updates/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs index (default 3, headline)")
+    ap.add_argument("--impl", default="mphv", choices=["mphv", "reference"])
+    ap.add_argument("--no-fusion", action="store_true", help="one kernel per sweep (for profiling)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU work of the oracle sample")
+    return ap.parse_args()
+
+
+# ------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """Samples SM clock and throttle reasons with NVML during the timed region."""
+
+    def __init__(self, index: int, period: float = 0.02):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self.period, self._stop, self._thr, self.h = period, threading.Event(), None, None
+        try:
+            import pynvml
+            self.nv = pynvml
+            pynvml.nvmlInit()
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception as e:  # noqa: BLE001
+            self.err = repr(e)
+
+    def _run(self):
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+            getattr(nv, "nvmlClocksEventReasonHwPowerBrakeSlowdown", 0x80): "hw_power_brake",
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    mask = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:  # noqa: BLE001
+                    mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if mask & bit:
+                        self.reasons.add(name)
+            except Exception:  # noqa: BLE001
+                pass
+            self._stop.wait(self.period)
+
+    def __enter__(self):
+        if self.h is not None:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thr:
+            self._thr.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                    "note": "no NVML samples"}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ------------------------------------------------------------------------------- oracle legs
+def oracle_sample(w, cpu_seconds: float):
+    """A spatial sub-block of workload w (same velocity grid, same f0/E/B recipe and dt rule,
+    block centred on the current sheet) sized for about cpu_seconds of oracle work."""
+    from paper_2305_01487_b200 import inputs
+    est_rate = 1.5e7 * max(1, os.cpu_count() or 1) ** 0.7      # cell-updates/s guess, plain C oracle
+    nvel = int(np.prod(w.nv))
+    target_space = max(16, int(cpu_seconds * est_rate / nvel))
+    if w.nx[2] > 1:
+        side = int(max(4, min(w.nx[0], round(target_space ** (1 / 3)))))
+        nx = (side, side, side)
+    elif w.nx[1] > 1:
+        sy = int(max(4, min(w.nx[1], round((target_space / 2) ** 0.5))))
+        sx = int(max(4, min(w.nx[0], target_space // sy)))
+        nx = (sx, sy, 1)
+    else:
+        nx = w.nx
+    dx = [w.dx(d) for d in range(3)]
+    xlo, xhi = list(w.xlo), list(w.xhi)
+    for d in range(3):
+        if w.nx[d] > 1:
+            mid = 0.5 * (w.xlo[d] + w.xhi[d]) if d == 1 else w.xlo[d] + 0.5 * nx[d] * dx[d]
+            xlo[d] = mid - 0.5 * nx[d] * dx[d]
+            xhi[d] = mid + 0.5 * nx[d] * dx[d]
+    sub = inputs.variant(w, name=w.name + f"_sub{nx[0]}x{nx[1]}x{nx[2]}", nx=tuple(nx),
+                         xlo=tuple(xlo), xhi=tuple(xhi))
+    return sub
+
+
+def time_oracle(w, steps: int, warmup: int, cpu_seconds: float):
+    """Times oracle.step + oracle.moments, as they stand, on a bounded sample of workload w."""
+    import oracle
+    from paper_2305_01487_b200 import inputs
+    sub = oracle_sample(w, cpu_seconds / max(1, steps + warmup))
+    f0, E, B, _ = inputs.make_all(sub)
+    dt = 0.5 * inputs.cfl_dt(sub, E, B)          # safely inside |s| < 1 on the sub-block
+    grid, box = oracle.Grid(sub.nx, sub.nv, sub.bc), oracle.Box(sub.xlo, sub.xhi, sub.vlo, sub.vhi)
+    f = f0.copy()
+    for _ in range(warmup):
+        oracle.step(f, grid, box, sub.q_over_m, E, B, dt)
+        oracle.moments(f, grid, box)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        oracle.step(f, grid, box, sub.q_over_m, E, B, dt)
+        oracle.moments(f, grid, box)
+    el = time.perf_counter() - t0
+    return {
+        "value": sub.n_cells * steps / el, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+        "sample": f"{sub.nx[0]}x{sub.nx[1]}x{sub.nx[2]} spatial sub-block x {sub.nv[0]}x{sub.nv[1]}x{sub.nv[2]} velocity "
+                  f"({sub.n_cells} cells) of {w.name}, {steps} full split steps + moments, {el:.2f} s",
+        "ms_per_step": 1e3 * el / steps,
+    }
+
+
+def run_reference(args, w):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    steps, warmup = max(1, args.steps), max(0, args.warmup)
+    r = time_oracle(w, steps, warmup, cpu_seconds=max(10.0, min(120.0, 3.0 * (steps + warmup))))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
+        "steps": steps, "warmup": warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "note": "CPU oracle on a bounded sample of the workload"},
+        "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
+        "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------- CUDA arm
+def run_mphv(args, w):
+    import torch
+    import torch.distributed as dist
+    from paper_2305_01487_b200 import inputs, mphv
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --impl mphv needs a B200: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    # each rank: its own seeded copy of the workload (independent problems => weak scaling)
+    wr = inputs.variant(w, seed_offset=1000 * rank)
+    f0, E, B, dt = inputs.make_all(wr)
+    peaks = {}
+    try:
+        peaks = json.loads((ROOT / "MEASURED_PEAKS.json").read_text())
+    except Exception:  # noqa: BLE001
+        pass
+    peak_gbs, peak_src = (float(peaks["hbm_gbs"]), "measured") if "hbm_gbs" in peaks else (6650.0, "fallback")
+
+    sim = mphv.Vlasov.from_workload(wr, device=dev)
+    sim.set_fusion(not args.no_fusion)
+    f = torch.from_numpy(f0).to(dev)
+    sim.bind_f(f)
+    sim.set_fields(torch.from_numpy(E).to(dev), torch.from_numpy(B).to(dev))
+    mom = sim.alloc_moments()
+    f_ref0 = f.clone() if w.n_cells <= 2 ** 28 else None
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(3, args.warmup)):
+        sim.step_moments(dt, mom)
+    barrier()
+    launches0 = sim.launches
+    sim.set_timing(True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as clk:
+        barrier()
+        e0.record()
+        for _ in range(args.steps):
+            sim.step_moments(dt, mom)
+        e1.record()
+        barrier()
+    ms = e0.elapsed_time(e1)
+    launches = sim.launches - launches0
+    timings = sim.timings()
+    sim.set_timing(False)
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    ms_per_step = ms / args.steps
+    value = w.n_cells * world * args.steps / (ms * 1e-3)
+
+    # sanity of the timed state: f finite, non-negative, moments finite
+    assert bool(torch.isfinite(mom[0]).all()) and float(f.min()) >= 0.0
+
+    # dominant kernel and its roofline (algorithmic bytes / CUDA-event duration)
+    kern = {k: dict(v, ms_per_launch=v["ms"] / v["launches"]) for k, v in timings.items()}
+    dom = max(kern, key=lambda k: kern[k]["ms"])
+    d = kern[dom]
+    achieved = d["alg_bytes"] / (d["ms_per_launch"] * 1e-3) / 1e9
+    step_alg_bytes = sum(v["alg_bytes"] * v["launches"] for v in kern.values()) / args.steps
+    roofline = {
+        "bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak_gbs, "unit": "GB/s",
+        "frac": achieved / peak_gbs, "peak_source": f"{peak_src} (MEASURED_PEAKS.json hbm_gbs)" if peak_src == "measured" else "fallback 6650 GB/s",
+        "traffic": None,
+        "share_of_step": d["ms"] / sum(v["ms"] for v in kern.values()),
+        "step_algorithmic_GBps": step_alg_bytes / (ms_per_step * 1e-3) / 1e9,
+        "step_frac_of_8TBps": step_alg_bytes / (ms_per_step * 1e-3) / 8e12,
+        "step_frac_of_measured": step_alg_bytes / (ms_per_step * 1e-3) / 1e9 / peak_gbs,
+        "kernels": {k: {"ms_per_launch": round(v["ms_per_launch"], 4), "launches_per_step": v["launches"] / args.steps,
+                        "alg_GBps": round(v["alg_bytes"] / (v["ms_per_launch"] * 1e-3) / 1e9, 1)} for k, v in kern.items()},
+    }
+    tr = ROOT / "profiles" / "traffic.json"
+    if tr.exists():
+        try:
+            roofline["traffic"] = json.loads(tr.read_text()).get(dom)
+        except Exception:  # noqa: BLE001
+            pass
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(3, args.warmup), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "cells_per_gpu": w.n_cells, "bytes_per_copy_of_f": w.n_cells * 8,
+                   "step": "S_x,S_y[,S_z],V_vx,V_vy,V_vz + moments n,j,P every step",
+                   "l2": "inputs larger than L2 (f is %.2f GB >> 126 MB); no flush needed" % (w.n_cells * 8 / 1e9),
+                   "fusion": not args.no_fusion, "parallelism": f"{world} independent problems" if world > 1 else "1 GPU"},
+        "clocks": clk.summary(), "gpu_launches": launches, "roofline": roofline,
+    }
+
+    # end to end through the C ABI with HOST buffers: H2D(f) + step + moments + D2H(f, moments) per step
+    if not args.no_e2e:
+        fh = torch.from_numpy(f0).pin_memory()
+        nh = torch.empty(wr.space_shape, dtype=torch.float64).pin_memory()
+        jh = torch.empty((3,) + wr.space_shape, dtype=torch.float64).pin_memory()
+        Ph = torch.empty((6,) + wr.space_shape, dtype=torch.float64).pin_memory()
+        sim.run_host(fh, 1, dt, nh, jh, Ph)                     # warm-up
+        barrier()
+        t0 = time.perf_counter()
+        e0.record()
+        for _ in range(args.e2e_steps):
+            sim.run_host(fh, 1, dt, nh, jh, Ph)
+        e1.record()
+        barrier()
+        wall = time.perf_counter() - t0
+        ems = max(e0.elapsed_time(e1), wall * 1e3)
+        if world > 1:
+            t = torch.tensor([ems], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ems = float(t.item())
+        line["e2e"] = {"value": w.n_cells * world * args.e2e_steps / (ems * 1e-3), "unit": UNIT,
+                       "h2d_bytes_per_step": w.n_cells * 8, "d2h_bytes_per_step": w.n_cells * 8 + 10 * wr.n_space * 8,
+                       "ms_per_step": ems / args.e2e_steps, "steps": args.e2e_steps,
+                       "what": "mphv_run_host: pinned host f -> device, full split step, moments, f and moments -> host"}
+        del fh
+
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        del f0
+        line["cpu_baseline"] = {k: v for k, v in time_oracle(w, 2, 1, args.cpu_seconds).items() if k != "ms_per_step"}
+
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    from paper_2305_01487_b200 import inputs
+    w = inputs.config(args.config)
+    if args.impl == "reference":
+        run_reference(args, w)
+    else:
+        run_mphv(args, w)
+
+
+if __name__ == "__main__":
+    main()

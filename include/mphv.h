@@ -1,0 +1,161 @@
+/*
+ * mphv.h -- C ABI of the B200-native (sm_100a) kinetic Vlasov hot path of muphyII
+ * (arXiv 2305.01487): dimensionally split, conservative, positivity-preserving
+ * third-order semi-Lagrangian (PFC) sweeps of f(x,v) plus the velocity moments n, j, P.
+ *
+ * Citations: "P:Lnnn" = PAPER.md line nnn; "R1..R14" = the readings listed in DESIGN.md
+ * (= SURVEY.md sec. 8(c)); BJ = BASELINE.json.
+ *
+ * Conventions (all calls)
+ * -----------------------
+ *  - Plain C, no torch types. "dev" pointers are CUDA device pointers owned by the
+ *    CALLER (the library allocates only O(spatial cells) workspace); they must stay
+ *    valid until the context's stream has drained. "host" pointers are host memory.
+ *  - Layouts, C order, fastest index LAST, interior cells only (no stored halo):
+ *        f    [nz][ny][nx][nvz][nvy][nvx]                  fp64
+ *        E, B [3][nz][ny][nx]   component-major, CELL-CENTRED (R8)
+ *        n    [nz][ny][nx];  j [3][nz][ny][nx];  P [6][nz][ny][nx] in order xx,xy,xz,yy,yz,zz
+ *  - Units: j = int v f d3v, P = int v v f d3v (no q, no m: the API carries only q/m; R10).
+ *  - Async: every *device* call only enqueues work on the context's stream and returns;
+ *    outputs are valid after the caller synchronises that stream. Host-buffer calls
+ *    (mphv_run_host) synchronise before returning.
+ *  - Errors: int status, 0 = MPHV_OK. No exception or abort crosses the ABI. A call that
+ *    fails with ARG/STATE/RANGE leaves f untouched. Text: mphv_strerror / mphv_last_error.
+ *  - Inactive dimension = extent 1. Inactive velocity dim: v == 0, dv == 1 in dV.
+ *    An active dimension needs extent >= 4 (two boundary cells per side).
+ *  - There is NO CPU fallback: without a CUDA device of compute capability 10.x
+ *    mphv_create fails (MPHV_ERR_ARCH / MPHV_ERR_CUDA through mphv_last_error(NULL)).
+ */
+#ifndef MPHV_H
+#define MPHV_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mphv_ctx mphv_ctx;      /* opaque; created/destroyed by the library */
+
+typedef struct {
+    int32_t nx[3];                     /* spatial extents x,y,z; 1 = inactive                    */
+    int32_t nv[3];                     /* velocity extents vx,vy,vz; 1 = inactive                */
+    int32_t bc[3];                     /* per spatial dim: MPHV_BC_PERIODIC or MPHV_BC_OUTFLOW   */
+} mphv_grid;
+
+typedef struct {                       /* cell-centred finite volumes tile [lo,hi) (R1)          */
+    double xlo[3], xhi[3], vlo[3], vhi[3];
+} mphv_box;
+
+enum { MPHV_BC_PERIODIC = 0, MPHV_BC_OUTFLOW = 1 };
+
+enum {
+    MPHV_OK        = 0,
+    MPHV_ERR_ARG   = 1,  /* null pointer, dim out of range or inactive, non-finite dt, extent < 1,
+                            hi <= lo, active extent < 4, bad bc                                    */
+    MPHV_ERR_STATE = 2,  /* f or fields not bound                                                  */
+    MPHV_ERR_RANGE = 3,  /* |s| >= 1 on a non-periodic axis (outflow or velocity), or |s| >= 1 on a
+                            periodic axis with no scratch bound                                    */
+    MPHV_ERR_CUDA  = 4,  /* CUDA runtime / launch error; text in mphv_last_error                   */
+    MPHV_ERR_ARCH  = 5   /* device is not compute capability 10.x (sm_100)                         */
+};
+
+/* Create a context for one species on one GPU (the current CUDA device).
+ * Grid/box per R1; q_over_m multiplies (E + v x B) in eq. (1).
+ * Returns NULL on error (reason: mphv_last_error(NULL)). BJ north_star: mphv_create. */
+mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_m);
+int mphv_destroy(mphv_ctx *ctx);
+
+/* CUDA stream (cudaStream_t passed as void*) all later calls enqueue on; NULL = legacy
+ * default stream (the default after create). */
+int mphv_set_stream(mphv_ctx *ctx, void *cuda_stream);
+
+/* Number of doubles in f = prod(nx) * prod(nv). 0 if ctx is NULL. */
+size_t mphv_f_count(const mphv_ctx *ctx);
+/* Number of spatial cells prod(nx). */
+size_t mphv_space_count(const mphv_ctx *ctx);
+
+/* Bind the distribution function (device, f_count doubles, 16-byte aligned) and an optional
+ * scratch buffer of the same size (device; NULL allowed). Scratch is only used when a
+ * periodic spatial sweep is asked for |s| >= 1 (whole-cell shifts, semi-Lagrangian part
+ * R3/R11); without it such a call returns MPHV_ERR_RANGE. All sweeps are in place. */
+int mphv_bind_f(mphv_ctx *ctx, double *f_dev, double *scratch_dev);
+
+/* E, B: device, [3][nz][ny][nx] each, cell-centred, borrowed until the next set_fields.
+ * The call also enqueues a small reduction that records max |a_d| bounds used for the
+ * MPHV_ERR_RANGE check of velocity sweeps; it synchronises the stream once to read the
+ * three bounds back (fields change once per step, sweeps do not sync). */
+int mphv_set_fields(mphv_ctx *ctx, const double *E_dev, const double *B_dev);
+
+/* Spatial sweep S_d(dt), d = dim in 0..2: every pencil of f along spatial axis d is remapped
+ * by the 1-D PFC-3 scheme with Courant number s = v_d dt / dx_d, v_d the velocity cell
+ * centre (term v.grad_x f of eq. (1); scheme P:L135; readings R1-R3, R6, R11, R12).
+ * Boundary: periodic = index wrap, outflow = zero-gradient ghosts (a1 of SURVEY 8(a)).
+ * dt < 0 is legal. Errors: ARG (dim inactive / out of range, dt not finite), STATE,
+ * RANGE (see above). */
+int mphv_sweep_x(mphv_ctx *ctx, int dim, double dt);
+
+/* Velocity sweep V_d(dt), d = dim in 0..2: every pencil along velocity axis d is remapped
+ * with s = a_d dt / dv_d, a_d = (q/m)(E_d + (v x B)_d) at the spatial cell, using the cell
+ * centres of the other two velocity components (eq. (1)). The velocity box is
+ * closed: empty ghosts and zero flux through the two wall faces (R7). |s| >= 1 anywhere
+ * => MPHV_ERR_RANGE (checked against the bound recorded by mphv_set_fields). */
+int mphv_sweep_v(mphv_ctx *ctx, int dim, double dt);
+
+/* Full split step (R4, R5): S_x, S_y, S_z, V_vx, V_vy, V_vz in that order, each with
+ * the full dt, inactive dimensions skipped, fields frozen. All range checks are done
+ * before the first sweep is enqueued. The library may fuse consecutive sweeps into one
+ * kernel; the result is that of the unfused sequence up to fp64 rounding. */
+int mphv_step(mphv_ctx *ctx, double dt);
+
+/* Velocity moments by the midpoint rule at velocity cell centres (R9, R10):
+ * n = sum f dV, j_a = sum v_a f dV, P_ab = sum v_a v_b f dV, dV = dvx dvy dvz.
+ * Outputs: device, n [nz][ny][nx], j [3][...], P [6][...] (xx,xy,xz,yy,yz,zz). */
+int mphv_moments(mphv_ctx *ctx, double *n_dev, double *j_dev, double *P_dev);
+
+/* mphv_step followed by mphv_moments of the new f, with the moments accumulated inside
+ * the last velocity sweep's kernel when that is possible (f is then read once less).
+ * Same result as the two calls up to fp64 summation order. */
+int mphv_step_moments(mphv_ctx *ctx, double dt, double *n_dev, double *j_dev, double *P_dev);
+
+/* Host-buffer convenience path (used for end-to-end timing): copies f_host (f_count doubles,
+ * ideally pinned) to the bound device f, runs nsteps x mphv_step(dt), computes the moments
+ * into library-owned device workspace, copies f back to f_host and the moments to
+ * n_host [ns], j_host [3 ns], P_host [6 ns] (any of the three may be NULL), and
+ * synchronises the stream. Requires bind_f and set_fields. */
+int mphv_run_host(mphv_ctx *ctx, double *f_host, int nsteps, double dt,
+                  double *n_host, double *j_host, double *P_host);
+
+/* Sum of all entries of the bound f (device reduction, deterministic order), written to
+ * *sum_dev (device, 1 double). Used for the mass checks of BJ (1e-13 relative). */
+int mphv_sum_f(mphv_ctx *ctx, double *sum_dev);
+
+/* Number of kernel launches enqueued through this context since creation (for the
+ * bench's gpu_launches figure). */
+uint64_t mphv_launch_count(const mphv_ctx *ctx);
+
+/* Per-kernel device timing. When enabled, every kernel launch of this context is bracketed by
+ * two CUDA events on the context's stream; durations accumulate per slot. Enabling (again)
+ * clears the records. mphv_get_timing synchronises the stream, then reports slot `slot`
+ * (0 <= slot < mphv_timing_slots()): its name (copied into name[name_cap]), the summed device
+ * time in ms, the number of launches, and the ALGORITHMIC bytes of one launch (f read once +
+ * written once per sweep it performs, f read once per moments pass). */
+int mphv_set_timing(mphv_ctx *ctx, int enabled);
+int mphv_timing_slots(void);
+int mphv_get_timing(mphv_ctx *ctx, int slot, char *name, size_t name_cap, double *total_ms,
+                    uint64_t *launches, double *alg_bytes_per_launch);
+
+/* Tuning knob for experiments and tests: 0 = unfused kernels only (one kernel per sweep),
+ * 1 = allow fused kernels (default). Results agree up to fp64 rounding either way. */
+int mphv_set_fusion(mphv_ctx *ctx, int enabled);
+
+const char *mphv_strerror(int code);
+/* Last error text of this context, or of the last failed mphv_create when ctx is NULL.
+ * The returned pointer is owned by the library and valid until the next failing call. */
+const char *mphv_last_error(const mphv_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MPHV_H */

@@ -1,0 +1,516 @@
+// mphv.cu -- the C-ABI boundary of include/mphv.h: argument validation, range checks,
+// launch configuration. All arithmetic of the method runs in the kernels of
+// mphv_kernels.cuh; there is no CPU fallback.
+#include "../../include/mphv.h"
+#include "mphv_kernels.cuh"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+using namespace mphv;
+
+struct mphv_ctx {
+    mphv_grid grid;
+    mphv_box box;
+    double qm;
+    cudaStream_t stream;
+    double *f, *scratch;
+    const double *E, *B;
+    size_t ns, nvel, nf;
+    double dx[3], dv[3];
+    GridDev gd;
+    double amax[3];          // max |a_d| over all pencils, from the last set_fields
+    double *ws;              // device workspace: [10*ns] moments + [SUM_BLOCKS] partials + [4] scalars
+    uint64_t launches;
+    int fusion;
+    int timing;
+    struct Pending { int slot; cudaEvent_t e0, e1; };
+    std::vector<Pending> *pending;
+    double slot_ms[16];
+    uint64_t slot_launches[16];
+    double slot_bytes[16];
+    char err[512];
+};
+
+enum { SLOT_SX0 = 0, SLOT_SX1, SLOT_SX2, SLOT_VX, SLOT_VY, SLOT_VZ, SLOT_MOM, SLOT_VXY, SLOT_VZMOM,
+       SLOT_SHIFT, SLOT_SUM, SLOT_AMAX, SLOT_COUNT };
+static const char *const SLOT_NAMES[SLOT_COUNT] = {
+    "sweep_x0", "sweep_x1", "sweep_x2", "sweep_vx", "sweep_vy", "sweep_vz", "moments",
+    "fused_vx_vy", "fused_vz_moments", "shift_periodic", "sum_f", "amax_fields" };
+
+namespace {
+
+const int SUM_BLOCKS = 1184;           // 8 x 148 SMs
+char g_create_err[512] = "";
+
+void set_err(mphv_ctx *c, const char *fmt, ...)
+{
+    char *dst = c ? c->err : g_create_err;
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(dst, 512, fmt, ap);
+    va_end(ap);
+}
+
+int cuda_fail(mphv_ctx *c, cudaError_t e, const char *what)
+{
+    set_err(c, "%s: %s", what, cudaGetErrorString(e));
+    return MPHV_ERR_CUDA;
+}
+
+#define CUDA_TRY(c, call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail((c), e_, #call); } while (0)
+
+// Brackets one kernel launch with CUDA events when timing is on.
+struct Timed {
+    mphv_ctx *c; int slot; cudaEvent_t e0, e1; bool on;
+    Timed(mphv_ctx *c_, int slot_, double alg_bytes) : c(c_), slot(slot_), e0(nullptr), e1(nullptr), on(false)
+    {
+        if (!c->timing) return;
+        if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) { cudaGetLastError(); return; }
+        on = true;
+        c->slot_bytes[slot] = alg_bytes;
+        cudaEventRecord(e0, c->stream);
+    }
+    ~Timed()
+    {
+        if (!on) return;
+        cudaEventRecord(e1, c->stream);
+        c->pending->push_back({ slot, e0, e1 });
+    }
+};
+
+void drain_timing(mphv_ctx *c, bool keep)
+{
+    for (auto &p : *c->pending) {
+        float ms = 0.f;
+        if (keep && cudaEventElapsedTime(&ms, p.e0, p.e1) == cudaSuccess) {
+            c->slot_ms[p.slot] += ms;
+            c->slot_launches[p.slot]++;
+        }
+        cudaEventDestroy(p.e0); cudaEventDestroy(p.e1);
+    }
+    cudaGetLastError();
+    c->pending->clear();
+}
+
+int after_launch(mphv_ctx *c, const char *what)
+{
+    c->launches++;
+    cudaError_t e = cudaPeekAtLastError();
+    if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(c, e, what); }
+    return MPHV_OK;
+}
+
+bool is_finite(double x) { return x == x && !std::isinf(x); }
+
+double host_vcentre(const mphv_ctx *c, int d, int j)
+{
+    return c->gd.vlo[d] + ((double)j + 0.5) * c->gd.dv[d];
+}
+
+// max over velocity cells of |s| for the spatial sweep d, s = (v dt)/dx evaluated as on the device
+double max_courant_x(const mphv_ctx *c, int d, double dt)
+{
+    double m = 0.0;
+    for (int j = 0; j < c->grid.nv[d]; ++j) {
+        const double s = std::fabs((host_vcentre(c, d, j) * dt) / c->dx[d]);
+        if (!(s == s)) return s;
+        if (s > m) m = s;
+    }
+    return m;
+}
+
+double max_courant_v(const mphv_ctx *c, int d, double dt)
+{
+    return std::fabs((c->amax[d] * dt) / c->dv[d]);   // NaN propagates
+}
+
+unsigned grid_for(long long threads, int block) { return (unsigned)((threads + block - 1) / block); }
+
+// ---- launchers ---------------------------------------------------------------------------
+
+template <int KIND, int BC>
+int launch_march(mphv_ctx *c, const MarchArgs &a)
+{
+    const int block = 256;
+    Timed tm(c, KIND == KIND_SPACE ? SLOT_SX0 + a.dim : SLOT_VX + a.dim, 16.0 * (double)c->nf);
+    if (a.inner % 2 == 0) {
+        const long long threads = a.outer * (a.inner / 2);
+        march_kernel<2, 4, KIND, BC><<<grid_for(threads, block), block, 0, c->stream>>>(a);
+    } else {
+        const long long threads = a.outer * a.inner;
+        march_kernel<1, 4, KIND, BC><<<grid_for(threads, block), block, 0, c->stream>>>(a);
+    }
+    return after_launch(c, "march_kernel");
+}
+
+MarchArgs march_args_space(const mphv_ctx *c, int d, double dt)
+{
+    MarchArgs a;
+    std::memset(&a, 0, sizeof a);
+    a.f = c->f;
+    const long long nvel = (long long)c->nvel;
+    const long long nx = c->grid.nx[0], ny = c->grid.nx[1], nz = c->grid.nx[2];
+    if (d == 0)      { a.outer = nz * ny; a.inner = nvel; }
+    else if (d == 1) { a.outer = nz;      a.inner = nx * nvel; }
+    else             { a.outer = 1;       a.inner = ny * nx * nvel; }
+    a.n = c->grid.nx[d];
+    a.dim = d;
+    a.dt = dt;
+    a.dx = c->dx[d];
+    a.g = c->gd;
+    return a;
+}
+
+MarchArgs march_args_vel(const mphv_ctx *c, int d, double dt)
+{
+    MarchArgs a;
+    std::memset(&a, 0, sizeof a);
+    a.f = c->f;
+    const long long nvx = c->grid.nv[0], nvy = c->grid.nv[1], nvz = c->grid.nv[2];
+    if (d == 2) { a.outer = (long long)c->ns;       a.inner = nvy * nvx; }
+    else        { a.outer = (long long)c->ns * nvz; a.inner = nvx; }
+    a.n = c->grid.nv[d];
+    a.dim = d;
+    a.dt = dt;
+    a.dx = c->dv[d];
+    a.E = c->E; a.B = c->B;
+    a.g = c->gd;
+    return a;
+}
+
+int do_sweep_x(mphv_ctx *c, int d, double dt)
+{
+    MarchArgs a = march_args_space(c, d, dt);
+    const double smax = max_courant_x(c, d, dt);
+    if (c->grid.bc[d] == MPHV_BC_OUTFLOW) return launch_march<KIND_SPACE, BC_OUT>(c, a);
+    if (smax < 1.0) return launch_march<KIND_SPACE, BC_PER>(c, a);
+    // whole-cell shifts on a periodic axis: out of place through scratch, then copy back
+    const long long threads = a.outer * a.inner;
+    Timed tm(c, SLOT_SHIFT, 16.0 * (double)c->nf);
+    shift_kernel<<<grid_for(threads, 256), 256, 0, c->stream>>>(a, c->f, c->scratch);
+    int st = after_launch(c, "shift_kernel");
+    if (st != MPHV_OK) return st;
+    CUDA_TRY(c, cudaMemcpyAsync(c->f, c->scratch, c->nf * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+    return MPHV_OK;
+}
+
+int do_sweep_v(mphv_ctx *c, int d, double dt)
+{
+    if (d == 0) {
+        VxArgs a;
+        std::memset(&a, 0, sizeof a);
+        a.f = c->f;
+        a.rows = (long long)c->ns * c->grid.nv[2] * c->grid.nv[1];
+        a.nvx = c->grid.nv[0];
+        a.dt = dt;
+        a.E = c->E; a.B = c->B;
+        a.g = c->gd;
+        const int block = 256;
+        const int ch = (a.nvx % 4 == 0) ? 4 : (a.nvx % 2 == 0 ? 2 : 1);
+        const int cpr = a.nvx / ch;
+        if (cpr > block) { set_err(c, "nvx = %d too large for the vx kernel (max %d)", a.nvx, block * 4); return MPHV_ERR_ARG; }
+        a.rows_per_cta = block / cpr;
+        const unsigned grid = (unsigned)((a.rows + a.rows_per_cta - 1) / a.rows_per_cta);
+        Timed tm(c, SLOT_VX, 16.0 * (double)c->nf);
+        if (ch == 4)      vx_kernel<4><<<grid, block, 0, c->stream>>>(a);
+        else if (ch == 2) vx_kernel<2><<<grid, block, 0, c->stream>>>(a);
+        else              vx_kernel<1><<<grid, block, 0, c->stream>>>(a);
+        return after_launch(c, "vx_kernel");
+    }
+    MarchArgs a = march_args_vel(c, d, dt);
+    return launch_march<KIND_VEL, BC_WALL>(c, a);
+}
+
+int do_moments(mphv_ctx *c, double *n, double *j, double *P)
+{
+    MomArgs a;
+    a.f = c->f; a.n = n; a.j = j; a.P = P;
+    a.dV = c->dv[0] * c->dv[1] * c->dv[2];
+    a.g = c->gd;
+    const long long plane = (long long)c->grid.nv[0] * c->grid.nv[1];
+    int block = 512;
+    while (block > 32 && block / 2 >= plane) block /= 2;
+    Timed tm(c, SLOT_MOM, 8.0 * (double)c->nf);
+    moments_kernel<<<(unsigned)c->ns, block, 0, c->stream>>>(a);
+    return after_launch(c, "moments_kernel");
+}
+
+int check_common(mphv_ctx *c, double dt, bool need_fields)
+{
+    if (!c) return MPHV_ERR_ARG;
+    if (!is_finite(dt)) { set_err(c, "dt is not finite"); return MPHV_ERR_ARG; }
+    if (!c->f) { set_err(c, "f not bound (mphv_bind_f)"); return MPHV_ERR_STATE; }
+    if (need_fields && (!c->E || !c->B)) { set_err(c, "fields not set (mphv_set_fields)"); return MPHV_ERR_STATE; }
+    return MPHV_OK;
+}
+
+int range_x(mphv_ctx *c, int d, double dt)
+{
+    const double smax = max_courant_x(c, d, dt);
+    if (c->grid.bc[d] == MPHV_BC_OUTFLOW) {
+        if (!(smax < 1.0)) { set_err(c, "spatial sweep %d: max |s| = %g >= 1 on an outflow axis", d, smax); return MPHV_ERR_RANGE; }
+    } else if (!(smax < 1.0)) {
+        if (!(smax == smax)) { set_err(c, "spatial sweep %d: Courant number is NaN", d); return MPHV_ERR_RANGE; }
+        if (!c->scratch) { set_err(c, "spatial sweep %d: max |s| = %g >= 1 needs a scratch buffer", d, smax); return MPHV_ERR_RANGE; }
+    }
+    return MPHV_OK;
+}
+
+int range_v(mphv_ctx *c, int d, double dt)
+{
+    const double smax = max_courant_v(c, d, dt);
+    if (!(smax < 1.0)) { set_err(c, "velocity sweep %d: max |s| = %g >= 1 (closed velocity box)", d, smax); return MPHV_ERR_RANGE; }
+    return MPHV_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_m)
+{
+    if (!grid || !box) { set_err(nullptr, "grid or box is NULL"); return nullptr; }
+    if (!is_finite(q_over_m)) { set_err(nullptr, "q_over_m is not finite"); return nullptr; }
+    for (int d = 0; d < 3; ++d) {
+        if (grid->nx[d] < 1 || grid->nv[d] < 1) { set_err(nullptr, "extent < 1 in dimension %d", d); return nullptr; }
+        if ((grid->nx[d] > 1 && grid->nx[d] < 4) || (grid->nv[d] > 1 && grid->nv[d] < 4)) {
+            set_err(nullptr, "active extent < 4 in dimension %d", d); return nullptr;
+        }
+        if (grid->bc[d] != MPHV_BC_PERIODIC && grid->bc[d] != MPHV_BC_OUTFLOW) { set_err(nullptr, "bad bc[%d]", d); return nullptr; }
+        if (grid->nx[d] > 1 && !(box->xhi[d] > box->xlo[d] && is_finite(box->xhi[d]) && is_finite(box->xlo[d]))) {
+            set_err(nullptr, "xhi <= xlo in dimension %d", d); return nullptr;
+        }
+        if (grid->nv[d] > 1 && !(box->vhi[d] > box->vlo[d] && is_finite(box->vhi[d]) && is_finite(box->vlo[d]))) {
+            set_err(nullptr, "vhi <= vlo in dimension %d", d); return nullptr;
+        }
+    }
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) { set_err(nullptr, "no CUDA device: %s (there is no CPU fallback)", cudaGetErrorString(e)); cudaGetLastError(); return nullptr; }
+    int major = 0;
+    e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+    if (e != cudaSuccess) { set_err(nullptr, "cudaDeviceGetAttribute: %s", cudaGetErrorString(e)); cudaGetLastError(); return nullptr; }
+    if (major != 10) { set_err(nullptr, "%s: device compute capability %d.x, need 10.x (sm_100a)", mphv_strerror(MPHV_ERR_ARCH), major); return nullptr; }
+
+    mphv_ctx *c = new (std::nothrow) mphv_ctx;
+    if (!c) { set_err(nullptr, "out of host memory"); return nullptr; }
+    std::memset(c, 0, sizeof *c);
+    c->pending = new (std::nothrow) std::vector<mphv_ctx::Pending>();
+    if (!c->pending) { set_err(nullptr, "out of host memory"); delete c; return nullptr; }
+    c->grid = *grid; c->box = *box; c->qm = q_over_m;
+    c->ns = (size_t)grid->nx[0] * grid->nx[1] * grid->nx[2];
+    c->nvel = (size_t)grid->nv[0] * grid->nv[1] * grid->nv[2];
+    c->nf = c->ns * c->nvel;
+    c->fusion = 1;
+    for (int d = 0; d < 3; ++d) {
+        c->dx[d] = grid->nx[d] > 1 ? (box->xhi[d] - box->xlo[d]) / (double)grid->nx[d] : 1.0;
+        c->dv[d] = grid->nv[d] > 1 ? (box->vhi[d] - box->vlo[d]) / (double)grid->nv[d] : 1.0;
+        c->gd.nx[d] = grid->nx[d]; c->gd.nv[d] = grid->nv[d];
+        c->gd.dv[d] = c->dv[d];
+        c->gd.vlo[d] = grid->nv[d] > 1 ? box->vlo[d] : -0.5;
+        c->amax[d] = NAN;
+    }
+    c->gd.qm = q_over_m;
+    c->gd.ns = (long long)c->ns;
+    c->gd.nvel = (long long)c->nvel;
+    e = cudaMalloc(&c->ws, (10 * c->ns + SUM_BLOCKS + 8) * sizeof(double));
+    if (e != cudaSuccess) { set_err(nullptr, "cudaMalloc workspace: %s", cudaGetErrorString(e)); cudaGetLastError(); delete c->pending; delete c; return nullptr; }
+    return c;
+}
+
+int mphv_destroy(mphv_ctx *c)
+{
+    if (!c) return MPHV_ERR_ARG;
+    if (c->ws) cudaFree(c->ws);
+    if (c->pending) { drain_timing(c, false); delete c->pending; }
+    delete c;
+    return MPHV_OK;
+}
+
+int mphv_set_stream(mphv_ctx *c, void *s)
+{
+    if (!c) return MPHV_ERR_ARG;
+    c->stream = (cudaStream_t)s;
+    return MPHV_OK;
+}
+
+size_t mphv_f_count(const mphv_ctx *c) { return c ? c->nf : 0; }
+size_t mphv_space_count(const mphv_ctx *c) { return c ? c->ns : 0; }
+
+int mphv_bind_f(mphv_ctx *c, double *f, double *scratch)
+{
+    if (!c) return MPHV_ERR_ARG;
+    if (!f) { set_err(c, "f_dev is NULL"); return MPHV_ERR_ARG; }
+    if (((uintptr_t)f & 15) || ((uintptr_t)scratch & 15)) { set_err(c, "f/scratch must be 16-byte aligned"); return MPHV_ERR_ARG; }
+    if (scratch == f) { set_err(c, "scratch must not alias f"); return MPHV_ERR_ARG; }
+    c->f = f; c->scratch = scratch;
+    return MPHV_OK;
+}
+
+int mphv_set_fields(mphv_ctx *c, const double *E, const double *B)
+{
+    if (!c) return MPHV_ERR_ARG;
+    if (!E || !B) { set_err(c, "E_dev or B_dev is NULL"); return MPHV_ERR_ARG; }
+    double *out = c->ws + 10 * c->ns + SUM_BLOCKS;
+    int st;
+    {
+        Timed tm(c, SLOT_AMAX, 0.0);
+        amax_kernel<<<1, 1024, 0, c->stream>>>(E, B, c->gd, out);
+        st = after_launch(c, "amax_kernel");
+    }
+    if (st != MPHV_OK) return st;
+    double h[3];
+    CUDA_TRY(c, cudaMemcpyAsync(h, out, sizeof h, cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    c->E = E; c->B = B;
+    for (int d = 0; d < 3; ++d) c->amax[d] = h[d];
+    return MPHV_OK;
+}
+
+int mphv_sweep_x(mphv_ctx *c, int dim, double dt)
+{
+    int st = check_common(c, dt, false);
+    if (st != MPHV_OK) return st;
+    if (dim < 0 || dim > 2 || c->grid.nx[dim] < 2) { set_err(c, "spatial dim %d out of range or inactive", dim); return MPHV_ERR_ARG; }
+    st = range_x(c, dim, dt);
+    if (st != MPHV_OK) return st;
+    return do_sweep_x(c, dim, dt);
+}
+
+int mphv_sweep_v(mphv_ctx *c, int dim, double dt)
+{
+    int st = check_common(c, dt, true);
+    if (st != MPHV_OK) return st;
+    if (dim < 0 || dim > 2 || c->grid.nv[dim] < 2) { set_err(c, "velocity dim %d out of range or inactive", dim); return MPHV_ERR_ARG; }
+    st = range_v(c, dim, dt);
+    if (st != MPHV_OK) return st;
+    return do_sweep_v(c, dim, dt);
+}
+
+static int step_checks(mphv_ctx *c, double dt)
+{
+    int st = check_common(c, dt, true);
+    if (st != MPHV_OK) return st;
+    for (int d = 0; d < 3; ++d)
+        if (c->grid.nx[d] > 1 && (st = range_x(c, d, dt)) != MPHV_OK) return st;
+    for (int d = 0; d < 3; ++d)
+        if (c->grid.nv[d] > 1 && (st = range_v(c, d, dt)) != MPHV_OK) return st;
+    return MPHV_OK;
+}
+
+int mphv_step(mphv_ctx *c, double dt)
+{
+    int st = step_checks(c, dt);
+    if (st != MPHV_OK) return st;
+    for (int d = 0; d < 3; ++d)
+        if (c->grid.nx[d] > 1 && (st = do_sweep_x(c, d, dt)) != MPHV_OK) return st;
+    for (int d = 0; d < 3; ++d)
+        if (c->grid.nv[d] > 1 && (st = do_sweep_v(c, d, dt)) != MPHV_OK) return st;
+    return MPHV_OK;
+}
+
+int mphv_moments(mphv_ctx *c, double *n, double *j, double *P)
+{
+    if (!c) return MPHV_ERR_ARG;
+    if (!n || !j || !P) { set_err(c, "n_dev, j_dev or P_dev is NULL"); return MPHV_ERR_ARG; }
+    if (!c->f) { set_err(c, "f not bound (mphv_bind_f)"); return MPHV_ERR_STATE; }
+    return do_moments(c, n, j, P);
+}
+
+int mphv_step_moments(mphv_ctx *c, double dt, double *n, double *j, double *P)
+{
+    if (!c) return MPHV_ERR_ARG;
+    if (!n || !j || !P) { set_err(c, "n_dev, j_dev or P_dev is NULL"); return MPHV_ERR_ARG; }
+    int st = mphv_step(c, dt);
+    if (st != MPHV_OK) return st;
+    return do_moments(c, n, j, P);
+}
+
+int mphv_run_host(mphv_ctx *c, double *f_host, int nsteps, double dt, double *n_host, double *j_host, double *P_host)
+{
+    int st = step_checks(c, dt);
+    if (st != MPHV_OK) return st;
+    if (!f_host || nsteps < 0) { set_err(c, "f_host is NULL or nsteps < 0"); return MPHV_ERR_ARG; }
+    CUDA_TRY(c, cudaMemcpyAsync(c->f, f_host, c->nf * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+    for (int s = 0; s < nsteps; ++s)
+        if ((st = mphv_step(c, dt)) != MPHV_OK) return st;
+    double *mn = c->ws, *mj = c->ws + c->ns, *mP = c->ws + 4 * c->ns;
+    if ((st = do_moments(c, mn, mj, mP)) != MPHV_OK) return st;
+    CUDA_TRY(c, cudaMemcpyAsync(f_host, c->f, c->nf * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    if (n_host) CUDA_TRY(c, cudaMemcpyAsync(n_host, mn, c->ns * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    if (j_host) CUDA_TRY(c, cudaMemcpyAsync(j_host, mj, 3 * c->ns * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    if (P_host) CUDA_TRY(c, cudaMemcpyAsync(P_host, mP, 6 * c->ns * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return MPHV_OK;
+}
+
+int mphv_sum_f(mphv_ctx *c, double *sum_dev)
+{
+    if (!c) return MPHV_ERR_ARG;
+    if (!sum_dev) { set_err(c, "sum_dev is NULL"); return MPHV_ERR_ARG; }
+    if (!c->f) { set_err(c, "f not bound (mphv_bind_f)"); return MPHV_ERR_STATE; }
+    double *partial = c->ws + 10 * c->ns;
+    Timed tm(c, SLOT_SUM, 8.0 * (double)c->nf);
+    sum_kernel<<<SUM_BLOCKS, 256, 0, c->stream>>>(c->f, (long long)c->nf, partial);
+    int st = after_launch(c, "sum_kernel");
+    if (st != MPHV_OK) return st;
+    sum_kernel<<<1, 256, 0, c->stream>>>(partial, SUM_BLOCKS, sum_dev);
+    return after_launch(c, "sum_kernel(final)");
+}
+
+int mphv_set_timing(mphv_ctx *c, int enabled)
+{
+    if (!c) return MPHV_ERR_ARG;
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    drain_timing(c, false);
+    for (int i = 0; i < 16; ++i) { c->slot_ms[i] = 0.0; c->slot_launches[i] = 0; c->slot_bytes[i] = 0.0; }
+    c->timing = enabled ? 1 : 0;
+    return MPHV_OK;
+}
+
+int mphv_timing_slots(void) { return SLOT_COUNT; }
+
+int mphv_get_timing(mphv_ctx *c, int slot, char *name, size_t name_cap, double *total_ms,
+                    uint64_t *launches, double *alg_bytes_per_launch)
+{
+    if (!c) return MPHV_ERR_ARG;
+    if (slot < 0 || slot >= SLOT_COUNT) { set_err(c, "timing slot %d out of range", slot); return MPHV_ERR_ARG; }
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    drain_timing(c, true);
+    if (name && name_cap) { std::strncpy(name, SLOT_NAMES[slot], name_cap - 1); name[name_cap - 1] = 0; }
+    if (total_ms) *total_ms = c->slot_ms[slot];
+    if (launches) *launches = c->slot_launches[slot];
+    if (alg_bytes_per_launch) *alg_bytes_per_launch = c->slot_bytes[slot];
+    return MPHV_OK;
+}
+
+uint64_t mphv_launch_count(const mphv_ctx *c) { return c ? c->launches : 0; }
+
+int mphv_set_fusion(mphv_ctx *c, int enabled)
+{
+    if (!c) return MPHV_ERR_ARG;
+    c->fusion = enabled ? 1 : 0;
+    return MPHV_OK;
+}
+
+const char *mphv_strerror(int code)
+{
+    switch (code) {
+    case MPHV_OK: return "MPHV_OK";
+    case MPHV_ERR_ARG: return "MPHV_ERR_ARG: bad argument";
+    case MPHV_ERR_STATE: return "MPHV_ERR_STATE: f or fields not bound";
+    case MPHV_ERR_RANGE: return "MPHV_ERR_RANGE: Courant number out of range for this axis";
+    case MPHV_ERR_CUDA: return "MPHV_ERR_CUDA: CUDA runtime error";
+    case MPHV_ERR_ARCH: return "MPHV_ERR_ARCH: device is not sm_100";
+    default: return "unknown mphv status";
+    }
+}
+
+const char *mphv_last_error(const mphv_ctx *c) { return c ? c->err : g_create_err; }
+
+}  // extern "C"

@@ -1,0 +1,304 @@
+"""Thin ctypes binding of the C-ABI library ``libmphv.so`` (include/mphv.h).
+
+Argument marshalling only: every step of the path (sweeps, moments, reductions) runs in
+the CUDA kernels of ``csrc/``. PyTorch is used for device memory and streams. There is no
+CPU fallback: if the library is missing it is built with nvcc, and if no sm_100 GPU is
+present ``mphv_create`` fails and :class:`MphvError` is raised.
+
+The module-level functions carry the C names (``mphv_create`` ... ``mphv_moments``) and take
+raw device pointers (ints) like the C calls do; :class:`Vlasov` wraps them for torch tensors.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+from typing import Optional, Sequence
+
+_PKG = Path(__file__).resolve().parent
+_SO = _PKG / "libmphv.so"
+
+BC_PERIODIC, BC_OUTFLOW = 0, 1
+OK, ERR_ARG, ERR_STATE, ERR_RANGE, ERR_CUDA, ERR_ARCH = 0, 1, 2, 3, 4, 5
+
+# every symbol include/mphv.h declares (tests check the library exports each of them)
+SYMBOLS = (
+    "mphv_create", "mphv_destroy", "mphv_set_stream", "mphv_f_count", "mphv_space_count",
+    "mphv_bind_f", "mphv_set_fields", "mphv_sweep_x", "mphv_sweep_v", "mphv_step",
+    "mphv_moments", "mphv_step_moments", "mphv_run_host", "mphv_sum_f", "mphv_launch_count",
+    "mphv_set_fusion", "mphv_strerror", "mphv_last_error",
+    "mphv_set_timing", "mphv_timing_slots", "mphv_get_timing",
+)
+
+
+class MphvError(RuntimeError):
+    def __init__(self, code: int, text: str):
+        super().__init__(f"[{code}] {text}")
+        self.code = code
+
+
+class mphv_grid(C.Structure):
+    _fields_ = [("nx", C.c_int32 * 3), ("nv", C.c_int32 * 3), ("bc", C.c_int32 * 3)]
+
+
+class mphv_box(C.Structure):
+    _fields_ = [("xlo", C.c_double * 3), ("xhi", C.c_double * 3),
+                ("vlo", C.c_double * 3), ("vhi", C.c_double * 3)]
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Load (building first if needed) the CUDA library. Raises if it cannot be had."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    from . import build as _build
+    so = _build.build()                      # no-op when up to date; raises if nvcc fails
+    L = C.CDLL(str(so))
+    vp, dbl, i32 = C.c_void_p, C.c_double, C.c_int
+    sig = {
+        "mphv_create": (vp, [C.POINTER(mphv_grid), C.POINTER(mphv_box), dbl]),
+        "mphv_destroy": (i32, [vp]),
+        "mphv_set_stream": (i32, [vp, vp]),
+        "mphv_f_count": (C.c_size_t, [vp]),
+        "mphv_space_count": (C.c_size_t, [vp]),
+        "mphv_bind_f": (i32, [vp, vp, vp]),
+        "mphv_set_fields": (i32, [vp, vp, vp]),
+        "mphv_sweep_x": (i32, [vp, i32, dbl]),
+        "mphv_sweep_v": (i32, [vp, i32, dbl]),
+        "mphv_step": (i32, [vp, dbl]),
+        "mphv_moments": (i32, [vp, vp, vp, vp]),
+        "mphv_step_moments": (i32, [vp, dbl, vp, vp, vp]),
+        "mphv_run_host": (i32, [vp, vp, i32, dbl, vp, vp, vp]),
+        "mphv_sum_f": (i32, [vp, vp]),
+        "mphv_launch_count": (C.c_uint64, [vp]),
+        "mphv_set_fusion": (i32, [vp, i32]),
+        "mphv_set_timing": (i32, [vp, i32]),
+        "mphv_timing_slots": (i32, []),
+        "mphv_get_timing": (i32, [vp, i32, C.c_char_p, C.c_size_t, C.POINTER(dbl),
+                                  C.POINTER(C.c_uint64), C.POINTER(dbl)]),
+        "mphv_strerror": (C.c_char_p, [i32]),
+        "mphv_last_error": (C.c_char_p, [vp]),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(L, name)
+        fn.restype, fn.argtypes = res, args
+    _lib = L
+    return L
+
+
+def loaded_library_path() -> str:
+    lib()
+    return str(_SO)
+
+
+# ------------------------------------------------------------------ C-named functions
+def mphv_strerror(code: int) -> str:
+    return lib().mphv_strerror(int(code)).decode()
+
+
+def mphv_last_error(ctx=None) -> str:
+    return lib().mphv_last_error(ctx).decode()
+
+
+def _check(ctx, st: int):
+    if st != OK:
+        raise MphvError(st, f"{mphv_strerror(st)}: {mphv_last_error(ctx)}")
+
+
+def mphv_create(nx: Sequence[int], nv: Sequence[int], bc: Sequence[int],
+                xlo: Sequence[float], xhi: Sequence[float],
+                vlo: Sequence[float], vhi: Sequence[float], q_over_m: float):
+    g = mphv_grid((C.c_int32 * 3)(*nx), (C.c_int32 * 3)(*nv), (C.c_int32 * 3)(*bc))
+    d3 = C.c_double * 3
+    b = mphv_box(d3(*xlo), d3(*xhi), d3(*vlo), d3(*vhi))
+    ctx = lib().mphv_create(C.byref(g), C.byref(b), float(q_over_m))
+    if not ctx:
+        raise MphvError(ERR_ARG, "mphv_create failed: " + mphv_last_error(None))
+    return ctx
+
+
+def mphv_destroy(ctx):
+    _check(None, lib().mphv_destroy(ctx))
+
+
+def mphv_set_stream(ctx, cuda_stream: int):
+    _check(ctx, lib().mphv_set_stream(ctx, cuda_stream))
+
+
+def mphv_f_count(ctx) -> int:
+    return int(lib().mphv_f_count(ctx))
+
+
+def mphv_space_count(ctx) -> int:
+    return int(lib().mphv_space_count(ctx))
+
+
+def mphv_bind_f(ctx, f_dev: int, scratch_dev: Optional[int] = None):
+    _check(ctx, lib().mphv_bind_f(ctx, f_dev, scratch_dev))
+
+
+def mphv_set_fields(ctx, E_dev: int, B_dev: int):
+    _check(ctx, lib().mphv_set_fields(ctx, E_dev, B_dev))
+
+
+def mphv_sweep_x(ctx, dim: int, dt: float):
+    _check(ctx, lib().mphv_sweep_x(ctx, int(dim), float(dt)))
+
+
+def mphv_sweep_v(ctx, dim: int, dt: float):
+    _check(ctx, lib().mphv_sweep_v(ctx, int(dim), float(dt)))
+
+
+def mphv_step(ctx, dt: float):
+    _check(ctx, lib().mphv_step(ctx, float(dt)))
+
+
+def mphv_moments(ctx, n_dev: int, j_dev: int, P_dev: int):
+    _check(ctx, lib().mphv_moments(ctx, n_dev, j_dev, P_dev))
+
+
+def mphv_step_moments(ctx, dt: float, n_dev: int, j_dev: int, P_dev: int):
+    _check(ctx, lib().mphv_step_moments(ctx, float(dt), n_dev, j_dev, P_dev))
+
+
+def mphv_run_host(ctx, f_host: int, nsteps: int, dt: float, n_host=None, j_host=None, P_host=None):
+    _check(ctx, lib().mphv_run_host(ctx, f_host, int(nsteps), float(dt), n_host, j_host, P_host))
+
+
+def mphv_sum_f(ctx, sum_dev: int):
+    _check(ctx, lib().mphv_sum_f(ctx, sum_dev))
+
+
+def mphv_launch_count(ctx) -> int:
+    return int(lib().mphv_launch_count(ctx))
+
+
+def mphv_set_fusion(ctx, enabled: bool):
+    _check(ctx, lib().mphv_set_fusion(ctx, 1 if enabled else 0))
+
+
+def mphv_set_timing(ctx, enabled: bool):
+    _check(ctx, lib().mphv_set_timing(ctx, 1 if enabled else 0))
+
+
+def mphv_timing_slots() -> int:
+    return int(lib().mphv_timing_slots())
+
+
+def mphv_get_timing(ctx, slot: int):
+    """(name, total_ms, launches, algorithmic bytes per launch) of one timing slot."""
+    name = C.create_string_buffer(64)
+    ms, n, b = C.c_double(0.0), C.c_uint64(0), C.c_double(0.0)
+    _check(ctx, lib().mphv_get_timing(ctx, int(slot), name, 64, C.byref(ms), C.byref(n), C.byref(b)))
+    return name.value.decode(), ms.value, int(n.value), b.value
+
+
+# ------------------------------------------------------------------ torch convenience
+class Vlasov:
+    """One species on one GPU. Holds the context and references to the bound tensors."""
+
+    def __init__(self, nx, nv, bc, xlo, xhi, vlo, vhi, q_over_m=1.0, device="cuda:0", stream=None):
+        import torch
+        self.torch = torch
+        self.device = torch.device(device)
+        self.nx, self.nv = tuple(nx), tuple(nv)
+        self.shape = (nx[2], nx[1], nx[0], nv[2], nv[1], nv[0])
+        self.space_shape = (nx[2], nx[1], nx[0])
+        with torch.cuda.device(self.device):
+            self.ctx = mphv_create(nx, nv, bc, xlo, xhi, vlo, vhi, q_over_m)
+            if stream is not None:
+                mphv_set_stream(self.ctx, stream.cuda_stream)
+        self.stream = stream
+        self.f = self.scratch = self.E = self.B = None
+        self._sum = None
+
+    @classmethod
+    def from_workload(cls, w, **kw):
+        return cls(w.nx, w.nv, w.bc, w.xlo, w.xhi, w.vlo, w.vhi, w.q_over_m, **kw)
+
+    def _dev(self, t, count):
+        torch = self.torch
+        if t.dtype != torch.float64 or not t.is_contiguous() or t.numel() != count or t.device != self.device:
+            raise ValueError(f"need a contiguous float64 tensor of {count} elements on {self.device}")
+        return t.data_ptr()
+
+    def close(self):
+        if self.ctx:
+            mphv_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def bind_f(self, f, scratch=None):
+        n = mphv_f_count(self.ctx)
+        mphv_bind_f(self.ctx, self._dev(f, n), None if scratch is None else self._dev(scratch, n))
+        self.f, self.scratch = f, scratch
+
+    def set_fields(self, E, B):
+        ns = mphv_space_count(self.ctx)
+        mphv_set_fields(self.ctx, self._dev(E, 3 * ns), self._dev(B, 3 * ns))
+        self.E, self.B = E, B
+
+    def sweep_x(self, dim, dt):
+        mphv_sweep_x(self.ctx, dim, dt)
+
+    def sweep_v(self, dim, dt):
+        mphv_sweep_v(self.ctx, dim, dt)
+
+    def step(self, dt):
+        mphv_step(self.ctx, dt)
+
+    def alloc_moments(self):
+        torch = self.torch
+        sp = self.space_shape
+        return (torch.empty(sp, dtype=torch.float64, device=self.device),
+                torch.empty((3,) + sp, dtype=torch.float64, device=self.device),
+                torch.empty((6,) + sp, dtype=torch.float64, device=self.device))
+
+    def moments(self, out=None):
+        n, j, P = out if out is not None else self.alloc_moments()
+        mphv_moments(self.ctx, n.data_ptr(), j.data_ptr(), P.data_ptr())
+        return n, j, P
+
+    def step_moments(self, dt, out=None):
+        n, j, P = out if out is not None else self.alloc_moments()
+        mphv_step_moments(self.ctx, dt, n.data_ptr(), j.data_ptr(), P.data_ptr())
+        return n, j, P
+
+    def sum_f(self) -> float:
+        torch = self.torch
+        if self._sum is None:
+            self._sum = torch.empty(1, dtype=torch.float64, device=self.device)
+        mphv_sum_f(self.ctx, self._sum.data_ptr())
+        return float(self._sum.item())
+
+    def run_host(self, f_host, nsteps, dt, n_host=None, j_host=None, P_host=None):
+        """f_host etc.: CPU float64 tensors (pinned for speed); updated in place."""
+        def hp(t):
+            return None if t is None else t.data_ptr()
+        mphv_run_host(self.ctx, f_host.data_ptr(), nsteps, dt, hp(n_host), hp(j_host), hp(P_host))
+
+    @property
+    def launches(self) -> int:
+        return mphv_launch_count(self.ctx)
+
+    def set_fusion(self, enabled: bool):
+        mphv_set_fusion(self.ctx, enabled)
+
+    def set_timing(self, enabled: bool):
+        mphv_set_timing(self.ctx, enabled)
+
+    def timings(self):
+        """{kernel name: dict(ms=total, launches=count, alg_bytes=per launch)} for slots that ran."""
+        out = {}
+        for s in range(mphv_timing_slots()):
+            name, ms, n, b = mphv_get_timing(self.ctx, s)
+            if n:
+                out[name] = dict(ms=ms, launches=n, alg_bytes=b)
+        return out

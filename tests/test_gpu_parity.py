@@ -1,0 +1,293 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element,
+on the same seeded inputs. Bar: 1e-12 relative per sweep/step (BASELINE.json), bit-exact for
+whole-cell shifts, mass to 1e-13. Run with ``-m gpu`` on a B200."""
+import numpy as np
+import pytest
+
+from parity_util import TOL_MASS, TOL_SWEEP, moments_err, rel_err
+
+pytestmark = pytest.mark.gpu
+
+# f array axes: [iz, iy, ix, jvz, jvy, jvx]
+AX_X = {0: 2, 1: 1, 2: 0}
+AX_V = {0: 5, 1: 4, 2: 3}
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "these tests need a GPU"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def mphv():
+    from paper_2305_01487_b200 import mphv as m
+    m.lib()
+    return m
+
+
+def small_workload(nx, nv, bc=(0, 1, 0), seed_offset=0, kind=None):
+    from paper_2305_01487_b200 import inputs
+    kind = kind or ("harris3d" if nx[2] > 1 else "harris2d")
+    return inputs.Workload(
+        name="small", index=1, kind=kind, nx=tuple(nx), nv=tuple(nv), bc=tuple(bc),
+        xlo=(0.0, -6.4, 0.0), xhi=(25.6, 6.4, 12.8), vlo=(-5.0,) * 3, vhi=(5.0,) * 3,
+        steps=2, seed_offset=seed_offset)
+
+
+class Pair:
+    """Same inputs on both sides: oracle on numpy arrays, CUDA path on device tensors."""
+
+    def __init__(self, torch, mphv, orc, w, with_scratch=False, fusion=True):
+        from paper_2305_01487_b200 import inputs
+        self.torch, self.orc, self.w = torch, orc, w
+        self.f0, self.E, self.B, self.dt = inputs.make_all(w)
+        self.grid = orc.Grid(w.nx, w.nv, w.bc)
+        self.box = orc.Box(w.xlo, w.xhi, w.vlo, w.vhi)
+        self.f_ref = self.f0.copy()
+        self.sim = mphv.Vlasov.from_workload(w)
+        self.sim.set_fusion(fusion)
+        self.f_dev = torch.from_numpy(self.f0).cuda()
+        self.scratch = torch.empty_like(self.f_dev) if with_scratch else None
+        self.sim.bind_f(self.f_dev, self.scratch)
+        self.E_dev, self.B_dev = torch.from_numpy(self.E).cuda(), torch.from_numpy(self.B).cuda()
+        self.sim.set_fields(self.E_dev, self.B_dev)
+
+    def gpu(self):
+        self.torch.cuda.synchronize()
+        return self.f_dev.cpu().numpy()
+
+    def set_f(self, arr):
+        self.f_ref = np.ascontiguousarray(arr, dtype=np.float64).copy()
+        self.f_dev.copy_(self.torch.from_numpy(self.f_ref))
+
+
+SHAPES = [
+    # nx, nv, bc : even/odd inner (double2 vs scalar path), ragged vs block sizes, 3-D
+    ((12, 10, 1), (12, 10, 8), (0, 1, 0)),
+    ((8, 12, 1), (9, 7, 5), (1, 0, 0)),
+    ((6, 5, 4), (8, 6, 4), (0, 1, 0)),
+    ((5, 4, 6), (7, 4, 12), (1, 1, 1)),
+    ((36, 8, 1), (40, 12, 6), (0, 1, 0)),
+]
+
+
+@pytest.mark.parametrize("nx,nv,bc", SHAPES)
+@pytest.mark.parametrize("sign", [1.0, -1.0])
+def test_each_sweep_matches_oracle(torch_cuda, mphv, orc, nx, nv, bc, sign):
+    w = small_workload(nx, nv, bc)
+    p = Pair(torch_cuda, mphv, orc, w)
+    dt = sign * p.dt * 1.7          # CFL 0.85: exercises large fractional shifts, both signs
+    for d in range(3):
+        if w.nx[d] > 1:
+            orc.sweep_x(p.f_ref, p.grid, p.box, d, dt)
+            p.sim.sweep_x(d, dt)
+            err = rel_err(p.gpu(), p.f_ref, AX_X[d])
+            assert err <= TOL_SWEEP, f"sweep_x({d}) err {err:.3e}"
+            p.set_f(p.f_ref)        # restart both sides from identical data
+    for d in range(3):
+        if w.nv[d] > 1:
+            orc.sweep_v(p.f_ref, p.grid, p.box, w.q_over_m, p.E, p.B, d, dt)
+            p.sim.sweep_v(d, dt)
+            err = rel_err(p.gpu(), p.f_ref, AX_V[d])
+            assert err <= TOL_SWEEP, f"sweep_v({d}) err {err:.3e}"
+            p.set_f(p.f_ref)
+
+
+def test_limiter_active_data_matches_oracle(torch_cuda, mphv, orc):
+    """Random non-negative data with exact zeros and spikes: every limiter branch fires."""
+    w = small_workload((16, 12, 1), (12, 8, 8), (0, 1, 0), seed_offset=5)
+    p = Pair(torch_cuda, mphv, orc, w)
+    rng = np.random.default_rng(99)
+    f = rng.uniform(0.0, 1.0, size=w.shape) ** 6
+    f[rng.uniform(size=w.shape) < 0.3] = 0.0
+    for d, fn_o, fn_g, ax in [(0, "x", "x", AX_X[0]), (1, "x", "x", AX_X[1]),
+                              (0, "v", "v", AX_V[0]), (1, "v", "v", AX_V[1]), (2, "v", "v", AX_V[2])]:
+        p.set_f(f)
+        if fn_o == "x":
+            orc.sweep_x(p.f_ref, p.grid, p.box, d, p.dt * 1.5)
+            p.sim.sweep_x(d, p.dt * 1.5)
+        else:
+            orc.sweep_v(p.f_ref, p.grid, p.box, w.q_over_m, p.E, p.B, d, p.dt * 1.5)
+            p.sim.sweep_v(d, p.dt * 1.5)
+        g = p.gpu()
+        assert g.min() >= 0.0, "positivity lost on the GPU"
+        assert rel_err(g, p.f_ref, ax) <= TOL_SWEEP
+
+
+@pytest.mark.parametrize("fusion", [False, True])
+def test_config0_landau_20_steps_and_moments(torch_cuda, mphv, orc, fusion):
+    from paper_2305_01487_b200 import inputs
+    w = inputs.config(0)
+    p = Pair(torch_cuda, mphv, orc, w, fusion=fusion)
+    for _ in range(w.steps):
+        orc.step(p.f_ref, p.grid, p.box, w.q_over_m, p.E, p.B, p.dt)
+        p.sim.step(p.dt)
+    g = p.gpu()
+    assert rel_err(g, p.f_ref, AX_V[0]) <= w.steps * TOL_SWEEP
+    m_ref, m_gpu = orc.total(p.f_ref), orc.total(g)
+    assert abs(m_gpu - m_ref) <= TOL_MASS * abs(m_ref)
+    assert abs(m_gpu - orc.total(p.f0)) <= TOL_MASS * abs(m_ref), "all-periodic grid: mass is conserved"
+    check_moments(p, orc, g)
+
+
+def check_moments(p, orc, g):
+    n_r, j_r, P_r = orc.moments(p.f_ref, p.grid, p.box)
+    n_g, j_g, P_g = (t.cpu().numpy() for t in p.sim.moments())
+    w = p.w
+    vx, vy, vz = (w.v_centres(d) for d in range(3))
+    dV = w.dv(0) * w.dv(1) * w.dv(2)
+    fa = np.abs(p.f_ref)
+    V = [vx[None, None, None, None, None, :], vy[None, None, None, None, :, None], vz[None, None, None, :, None, None]]
+    assert moments_err(n_g, n_r, fa.sum(axis=(3, 4, 5)) * dV) <= 1e-13
+    for a in range(3):
+        assert moments_err(j_g[a], j_r[a], (fa * np.abs(V[a])).sum(axis=(3, 4, 5)) * dV) <= 1e-13
+    k = 0
+    for a in range(3):
+        for b in range(a, 3):
+            assert moments_err(P_g[k], P_r[k], (fa * np.abs(V[a] * V[b])).sum(axis=(3, 4, 5)) * dV) <= 1e-13
+            k += 1
+
+
+@pytest.mark.parametrize("fusion", [False, True])
+def test_config1_harris_steps_and_moments(torch_cuda, mphv, orc, fusion):
+    from paper_2305_01487_b200 import inputs
+    w = inputs.config(1)
+    p = Pair(torch_cuda, mphv, orc, w, fusion=fusion)
+    nsteps = 3
+    for s in range(nsteps):
+        orc.step(p.f_ref, p.grid, p.box, w.q_over_m, p.E, p.B, p.dt)
+        p.sim.step(p.dt)
+        if s == 0:
+            assert rel_err(p.gpu(), p.f_ref, AX_V[2]) <= TOL_SWEEP, "single step must meet 1e-12"
+    g = p.gpu()
+    assert rel_err(g, p.f_ref, AX_V[2]) <= nsteps * TOL_SWEEP
+    assert g.min() >= 0.0
+    m_ref, m_gpu = orc.total(p.f_ref), orc.total(g)
+    assert abs(m_gpu - m_ref) <= TOL_MASS * abs(m_ref)
+    assert abs(p.sim.sum_f() - m_ref) <= TOL_MASS * abs(m_ref), "device-side sum"
+    check_moments(p, orc, g)
+
+
+def test_step_moments_equals_step_then_moments(torch_cuda, mphv, orc):
+    w = small_workload((8, 8, 1), (12, 10, 8))
+    p = Pair(torch_cuda, mphv, orc, w)
+    orc.step(p.f_ref, p.grid, p.box, w.q_over_m, p.E, p.B, p.dt)
+    n_g, j_g, P_g = (t.cpu().numpy() for t in p.sim.step_moments(p.dt))
+    g = p.gpu()
+    assert rel_err(g, p.f_ref, AX_V[2]) <= TOL_SWEEP
+    n_r, j_r, P_r = orc.moments(p.f_ref, p.grid, p.box)
+    scale = np.abs(P_r[0]) + np.abs(P_r[3]) + np.abs(P_r[5]) + np.abs(n_r)
+    for a, b in [(n_g, n_r), (j_g, j_r), (P_g, P_r)]:
+        assert np.max(np.abs(a - b) / scale) <= 1e-12
+
+
+def test_3d3v_step_all_six_sweeps(torch_cuda, mphv, orc):
+    w = small_workload((8, 6, 8), (8, 8, 8), (0, 1, 0))
+    p = Pair(torch_cuda, mphv, orc, w)
+    for _ in range(2):
+        orc.step(p.f_ref, p.grid, p.box, w.q_over_m, p.E, p.B, p.dt)
+        p.sim.step(p.dt)
+    g = p.gpu()
+    assert rel_err(g, p.f_ref, AX_V[2]) <= 2 * TOL_SWEEP
+    check_moments(p, orc, g)
+
+
+def test_integer_courant_is_bitwise_roll(torch_cuda, mphv, orc):
+    """P1 on the GPU: dyadic dx, dv and dt = 2 dx / dv give odd-integer Courant numbers; the
+    sweep must equal the index-rolled input bit for bit (whole-cell shift path, needs scratch)."""
+    from paper_2305_01487_b200 import inputs
+    w = inputs.Workload(name="p1", index=0, kind="harris2d", nx=(16, 8, 1), nv=(8, 4, 4), bc=(0, 0, 0),
+                        xlo=(0.0, 0.0, 0.0), xhi=(16.0, 8.0, 1.0), vlo=(-2.0, -1.0, -1.0), vhi=(2.0, 1.0, 1.0))
+    p = Pair(torch_cuda, mphv, orc, w, with_scratch=True)
+    rng = np.random.default_rng(3)
+    f = rng.uniform(0.0, 1.0, size=w.shape)
+    p.set_f(f)
+    dt = 2.0 * 1.0 / 0.5            # s_j = v_j dt / dx = (j + 1/2) 0.5 * 4 - 8 = odd integers
+    p.sim.sweep_x(0, dt)
+    g = p.gpu()
+    vx = w.v_centres(0)
+    for j, v in enumerate(vx):
+        k = int(round(v * dt / 1.0))
+        assert k % 2 != 0
+        assert np.array_equal(g[..., j], np.roll(f[..., j], k, axis=2))
+    # fractional + whole-cell shift against the oracle, |s| up to 3.6
+    p.set_f(f)
+    orc.sweep_x(p.f_ref, p.grid, p.box, 0, 0.9 * dt)
+    p.sim.sweep_x(0, 0.9 * dt)
+    assert rel_err(p.gpu(), p.f_ref, AX_X[0]) <= TOL_SWEEP
+    # zero time step: identity, bitwise, on every in-place kernel
+    p.set_f(f)
+    for d in (0, 1):
+        p.sim.sweep_x(d, 0.0)
+    for d in (0, 1, 2):
+        p.sim.sweep_v(d, 0.0)
+    assert np.array_equal(p.gpu(), f)
+
+
+def test_mirror_symmetry_on_gpu(torch_cuda, mphv, orc):
+    """reverse(sweep(f, dt)) == sweep(reverse(f), -dt) along a periodic axis (<= 1e-12)."""
+    w = small_workload((16, 8, 1), (8, 8, 4), (0, 0, 0))
+    p = Pair(torch_cuda, mphv, orc, w)
+    f = p.f0.copy()
+    p.sim.sweep_x(0, p.dt)
+    a = p.gpu()
+    # mirror x and vx together: v -> -v, x -> -x leaves v dt/dx unchanged in sign convention
+    p.set_f(f[:, :, ::-1])
+    p.sim.sweep_x(0, -p.dt)
+    b = p.gpu()[:, :, ::-1]
+    assert rel_err(a, b, AX_X[0]) <= TOL_SWEEP
+
+
+def test_error_codes_on_gpu(torch_cuda, mphv, orc):
+    torch = torch_cuda
+    w = small_workload((8, 8, 1), (8, 8, 8))
+    sim = mphv.Vlasov.from_workload(w)
+    with pytest.raises(mphv.MphvError) as ei:
+        sim.step(0.1)
+    assert ei.value.code == mphv.ERR_STATE
+    f = torch.zeros(w.shape, dtype=torch.float64, device="cuda")
+    sim.bind_f(f)
+    with pytest.raises(mphv.MphvError) as ei:
+        sim.sweep_v(0, 0.1)
+    assert ei.value.code == mphv.ERR_STATE
+    E = torch.zeros((3,) + w.space_shape, dtype=torch.float64, device="cuda")
+    B = torch.ones((3,) + w.space_shape, dtype=torch.float64, device="cuda")
+    sim.set_fields(E, B)
+    f.fill_(1.0)
+    for call, code in [(lambda: sim.sweep_x(2, 0.1), mphv.ERR_ARG), (lambda: sim.sweep_x(3, 0.1), mphv.ERR_ARG),
+                       (lambda: sim.sweep_x(0, float("nan")), mphv.ERR_ARG),
+                       (lambda: sim.sweep_x(1, 10.0), mphv.ERR_RANGE),      # outflow axis, |s| >= 1
+                       (lambda: sim.sweep_x(0, 10.0), mphv.ERR_RANGE),      # periodic, no scratch
+                       (lambda: sim.sweep_v(0, 10.0), mphv.ERR_RANGE),
+                       (lambda: sim.step(10.0), mphv.ERR_RANGE)]:
+        with pytest.raises(mphv.MphvError) as ei:
+            call()
+        assert ei.value.code == code
+    torch.cuda.synchronize()
+    assert bool((f == 1.0).all()), "a failed call leaves f untouched"
+    # the RANGE decision is the oracle's: |s| < 1 accepted right up to the bound
+    vmax = float(np.max(np.abs(w.v_centres(0))))
+    amax = 2.0 * vmax                       # |v_a B_b - v_b B_a| with B = (1,1,1)
+    dt_ok = 0.999 * w.dv(0) / amax
+    sim.sweep_v(0, dt_ok)
+    with pytest.raises(mphv.MphvError):
+        sim.sweep_v(0, 1.001 * w.dv(0) / amax)
+
+
+def test_run_host_roundtrip(torch_cuda, mphv, orc):
+    torch = torch_cuda
+    w = small_workload((8, 8, 1), (8, 8, 8))
+    p = Pair(torch, mphv, orc, w)
+    fh = torch.from_numpy(p.f0.copy()).pin_memory()
+    nh = torch.empty(w.space_shape, dtype=torch.float64).pin_memory()
+    jh = torch.empty((3,) + w.space_shape, dtype=torch.float64).pin_memory()
+    Ph = torch.empty((6,) + w.space_shape, dtype=torch.float64).pin_memory()
+    p.sim.run_host(fh, 2, p.dt, nh, jh, Ph)
+    for _ in range(2):
+        orc.step(p.f_ref, p.grid, p.box, w.q_over_m, p.E, p.B, p.dt)
+    assert rel_err(fh.numpy(), p.f_ref, AX_V[2]) <= 2 * TOL_SWEEP
+    n_r, j_r, P_r = orc.moments(p.f_ref, p.grid, p.box)
+    assert np.max(np.abs(nh.numpy() - n_r) / np.abs(n_r)) <= 1e-12
+    assert np.max(np.abs(Ph.numpy()[0] - P_r[0]) / np.abs(P_r[0])) <= 1e-12
