@@ -24,7 +24,10 @@ struct mphv_ctx {
     double dx[3], dv[3];
     GridDev gd;
     double amax[3];          // max |a_d| over all pencils, from the last set_fields
-    double *ws;              // device workspace: [10*ns] moments + [SUM_BLOCKS] partials + [4] scalars
+    double *ws;              // device workspace: [10 ns] moments | [10 ns mom_tiles] partials | [SUM_BLOCKS] | [8]
+    int mom_tiles, mom_per_tile, mom_block;   // CTA tiling of the fused V_vz + moments kernel
+    int sm_count;
+    int vxy_T, vxy_grid; size_t vxy_smem;     // fused V_vx + V_vy plane kernel launch shape (0 = unsupported)
     uint64_t launches;
     int fusion;
     int timing;
@@ -140,12 +143,52 @@ int launch_march(mphv_ctx *c, const MarchArgs &a)
     Timed tm(c, KIND == KIND_SPACE ? SLOT_SX0 + a.dim : SLOT_VX + a.dim, 16.0 * (double)c->nf);
     if (a.inner % 2 == 0) {
         const long long threads = a.outer * (a.inner / 2);
-        march_kernel<2, 4, KIND, BC><<<grid_for(threads, block), block, 0, c->stream>>>(a);
+        march_kernel<2, 4, KIND, BC, false><<<grid_for(threads, block), block, 0, c->stream>>>(a);
     } else {
         const long long threads = a.outer * a.inner;
-        march_kernel<1, 4, KIND, BC><<<grid_for(threads, block), block, 0, c->stream>>>(a);
+        march_kernel<1, 4, KIND, BC, false><<<grid_for(threads, block), block, 0, c->stream>>>(a);
     }
     return after_launch(c, "march_kernel");
+}
+
+double *ws_moments(mphv_ctx *c) { return c->ws; }
+double *ws_partials(mphv_ctx *c) { return c->ws + 10 * c->ns; }
+double *ws_sum(mphv_ctx *c) { return c->ws + 10 * c->ns * (1 + (size_t)c->mom_tiles); }
+double *ws_scalars(mphv_ctx *c) { return ws_sum(c) + SUM_BLOCKS; }
+
+// V_vz with the moments of the new f accumulated in the same kernel (f read once less)
+int launch_vz_moments(mphv_ctx *c, MarchArgs a, double *n, double *j, double *P)
+{
+    Timed tm(c, SLOT_VZMOM, 24.0 * (double)c->nf);
+    a.mom = ws_partials(c);
+    a.tiles = c->mom_tiles;
+    a.per_tile = c->mom_per_tile;
+    a.dV = c->dv[0] * c->dv[1] * c->dv[2];
+    const unsigned grid = (unsigned)(c->ns * (size_t)c->mom_tiles);
+    if (a.inner % 2 == 0) march_kernel<2, 4, KIND_VEL, BC_WALL, true><<<grid, c->mom_block, 0, c->stream>>>(a);
+    else                  march_kernel<1, 4, KIND_VEL, BC_WALL, true><<<grid, c->mom_block, 0, c->stream>>>(a);
+    int st = after_launch(c, "march_kernel(vz+moments)");
+    if (st != MPHV_OK) return st;
+    mom_finalize_kernel<<<grid_for((long long)c->ns * 10, 256), 256, 0, c->stream>>>(a.mom, c->mom_tiles, (long long)c->ns, a.dV, n, j, P);
+    return after_launch(c, "mom_finalize_kernel");
+}
+
+int launch_vxy(mphv_ctx *c, double dt)
+{
+    PlaneArgs a;
+    std::memset(&a, 0, sizeof a);
+    a.f = c->f;
+    a.planes = (long long)c->ns * c->grid.nv[2];
+    a.nvx = c->grid.nv[0]; a.nvy = c->grid.nv[1]; a.nvz = c->grid.nv[2];
+    a.hx = a.nvx / 2; a.hy = a.nvy / 2;
+    a.inv_hx = 1.0f / (float)a.hx;
+    a.dt = dt;
+    a.E = c->E; a.B = c->B;
+    a.g = c->gd;
+    Timed tm(c, SLOT_VXY, 32.0 * (double)c->nf);
+    const long long grid = a.planes < c->vxy_grid ? a.planes : c->vxy_grid;
+    vxy_kernel<3><<<(unsigned)grid, c->vxy_T, c->vxy_smem, c->stream>>>(a);
+    return after_launch(c, "vxy_kernel");
 }
 
 MarchArgs march_args_space(const mphv_ctx *c, int d, double dt)
@@ -224,6 +267,26 @@ int do_sweep_v(mphv_ctx *c, int d, double dt)
     }
     MarchArgs a = march_args_vel(c, d, dt);
     return launch_march<KIND_VEL, BC_WALL>(c, a);
+}
+
+int do_moments(mphv_ctx *c, double *n, double *j, double *P);
+
+// The whole V stage (active velocity sweeps in order vx, vy, vz) and, if n != NULL, the moments
+// of the result. With fusion on: [vx+vy in one plane kernel], [vz + moments in one kernel].
+int do_v_stage(mphv_ctx *c, double dt, double *n, double *j, double *P)
+{
+    int st;
+    const bool ax = c->grid.nv[0] > 1, ay = c->grid.nv[1] > 1, az = c->grid.nv[2] > 1;
+    if (c->fusion && ax && ay && c->vxy_T > 0) {
+        if ((st = launch_vxy(c, dt)) != MPHV_OK) return st;
+    } else {
+        if (ax && (st = do_sweep_v(c, 0, dt)) != MPHV_OK) return st;
+        if (ay && (st = do_sweep_v(c, 1, dt)) != MPHV_OK) return st;
+    }
+    if (az && n && c->fusion) return launch_vz_moments(c, march_args_vel(c, 2, dt), n, j, P);
+    if (az && (st = do_sweep_v(c, 2, dt)) != MPHV_OK) return st;
+    if (n) return do_moments(c, n, j, P);
+    return MPHV_OK;
 }
 
 int do_moments(mphv_ctx *c, double *n, double *j, double *P)
@@ -318,7 +381,34 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
     c->gd.qm = q_over_m;
     c->gd.ns = (long long)c->ns;
     c->gd.nvel = (long long)c->nvel;
-    e = cudaMalloc(&c->ws, (10 * c->ns + SUM_BLOCKS + 8) * sizeof(double));
+    {   // CTA tiling of the fused V_vz + moments kernel: tiles of <= 256 (vector) pencils per spatial cell
+        const long long plane = (long long)grid->nv[0] * grid->nv[1];
+        const long long innerV = plane % 2 == 0 ? plane / 2 : plane;
+        c->mom_tiles = (int)((innerV + 255) / 256);
+        c->mom_per_tile = (int)((innerV + c->mom_tiles - 1) / c->mom_tiles);
+        c->mom_block = ((c->mom_per_tile + 31) / 32) * 32;
+    }
+    cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    c->vxy_T = 0;
+    if (grid->nv[0] >= 4 && grid->nv[1] >= 4 && grid->nv[0] % 2 == 0 && grid->nv[1] % 2 == 0) {
+        const int nvx = grid->nv[0], nvy = grid->nv[1];
+        int T = ((nvx / 2) * (nvy / 2) + 31) / 32 * 32;
+        const int T2 = (nvx + nvy + 31) / 32 * 32;
+        if (T < T2) T = T2;
+        if (T > 448) T = 448;
+        const size_t smem = ((size_t)(3 + 1) * nvx * nvy + 6 * (size_t)(nvx + nvy) + 3) * sizeof(double);
+        int max_optin = 0;
+        cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+        if (nvx + nvy <= T && smem <= (size_t)max_optin &&
+            cudaFuncSetAttribute(vxy_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess) {
+            int per_sm = 0;
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, vxy_kernel<3>, T, smem) == cudaSuccess && per_sm > 0) {
+                c->vxy_T = T; c->vxy_smem = smem; c->vxy_grid = per_sm * c->sm_count;
+            }
+        }
+        cudaGetLastError();
+    }
+    e = cudaMalloc(&c->ws, (10 * c->ns * (1 + (size_t)c->mom_tiles) + SUM_BLOCKS + 8) * sizeof(double));
     if (e != cudaSuccess) { set_err(nullptr, "cudaMalloc workspace: %s", cudaGetErrorString(e)); cudaGetLastError(); delete c->pending; delete c; return nullptr; }
     return c;
 }
@@ -356,7 +446,7 @@ int mphv_set_fields(mphv_ctx *c, const double *E, const double *B)
 {
     if (!c) return MPHV_ERR_ARG;
     if (!E || !B) { set_err(c, "E_dev or B_dev is NULL"); return MPHV_ERR_ARG; }
-    double *out = c->ws + 10 * c->ns + SUM_BLOCKS;
+    double *out = ws_scalars(c);
     int st;
     {
         Timed tm(c, SLOT_AMAX, 0.0);
@@ -403,16 +493,16 @@ static int step_checks(mphv_ctx *c, double dt)
     return MPHV_OK;
 }
 
-int mphv_step(mphv_ctx *c, double dt)
+static int step_impl(mphv_ctx *c, double dt, double *n, double *j, double *P)
 {
     int st = step_checks(c, dt);
     if (st != MPHV_OK) return st;
     for (int d = 0; d < 3; ++d)
         if (c->grid.nx[d] > 1 && (st = do_sweep_x(c, d, dt)) != MPHV_OK) return st;
-    for (int d = 0; d < 3; ++d)
-        if (c->grid.nv[d] > 1 && (st = do_sweep_v(c, d, dt)) != MPHV_OK) return st;
-    return MPHV_OK;
+    return do_v_stage(c, dt, n, j, P);
 }
+
+int mphv_step(mphv_ctx *c, double dt) { return step_impl(c, dt, nullptr, nullptr, nullptr); }
 
 int mphv_moments(mphv_ctx *c, double *n, double *j, double *P)
 {
@@ -426,9 +516,7 @@ int mphv_step_moments(mphv_ctx *c, double dt, double *n, double *j, double *P)
 {
     if (!c) return MPHV_ERR_ARG;
     if (!n || !j || !P) { set_err(c, "n_dev, j_dev or P_dev is NULL"); return MPHV_ERR_ARG; }
-    int st = mphv_step(c, dt);
-    if (st != MPHV_OK) return st;
-    return do_moments(c, n, j, P);
+    return step_impl(c, dt, n, j, P);
 }
 
 int mphv_run_host(mphv_ctx *c, double *f_host, int nsteps, double dt, double *n_host, double *j_host, double *P_host)
@@ -437,10 +525,12 @@ int mphv_run_host(mphv_ctx *c, double *f_host, int nsteps, double dt, double *n_
     if (st != MPHV_OK) return st;
     if (!f_host || nsteps < 0) { set_err(c, "f_host is NULL or nsteps < 0"); return MPHV_ERR_ARG; }
     CUDA_TRY(c, cudaMemcpyAsync(c->f, f_host, c->nf * sizeof(double), cudaMemcpyHostToDevice, c->stream));
-    for (int s = 0; s < nsteps; ++s)
+    double *mn = ws_moments(c), *mj = mn + c->ns, *mP = mn + 4 * c->ns;
+    for (int s = 0; s + 1 < nsteps; ++s)
         if ((st = mphv_step(c, dt)) != MPHV_OK) return st;
-    double *mn = c->ws, *mj = c->ws + c->ns, *mP = c->ws + 4 * c->ns;
-    if ((st = do_moments(c, mn, mj, mP)) != MPHV_OK) return st;
+    if (nsteps > 0) st = step_impl(c, dt, mn, mj, mP);       // last step with the moments fused in
+    else st = do_moments(c, mn, mj, mP);
+    if (st != MPHV_OK) return st;
     CUDA_TRY(c, cudaMemcpyAsync(f_host, c->f, c->nf * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     if (n_host) CUDA_TRY(c, cudaMemcpyAsync(n_host, mn, c->ns * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     if (j_host) CUDA_TRY(c, cudaMemcpyAsync(j_host, mj, 3 * c->ns * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
@@ -454,7 +544,7 @@ int mphv_sum_f(mphv_ctx *c, double *sum_dev)
     if (!c) return MPHV_ERR_ARG;
     if (!sum_dev) { set_err(c, "sum_dev is NULL"); return MPHV_ERR_ARG; }
     if (!c->f) { set_err(c, "f not bound (mphv_bind_f)"); return MPHV_ERR_STATE; }
-    double *partial = c->ws + 10 * c->ns;
+    double *partial = ws_sum(c);
     Timed tm(c, SLOT_SUM, 8.0 * (double)c->nf);
     sum_kernel<<<SUM_BLOCKS, 256, 0, c->stream>>>(c->f, (long long)c->nf, partial);
     int st = after_launch(c, "sum_kernel");

@@ -42,7 +42,8 @@ struct MarchArgs {
     double dt;
     double dx;              // width of the swept cell (dx_d or dv_d)
     const double *E, *B;    // velocity sweeps only
-    double *mom;            // fused moments output workspace [10][ns] (vz sweep only) or null
+    double *mom;            // fused moments: per-CTA partials [ns*tiles][10] (vz sweep only) or null
+    int tiles, per_tile;    // CTA tiling of the fused-moments variant
     double dV;
     GridDev g;
 };
@@ -77,8 +78,8 @@ __device__ __forceinline__ double face_flux(double a, double b, double c, double
     const double dp = c - b;
     const double dm = b - a;
     const double cap = b + b;
-    const double lp = dp > 0.0 ? fmin(dp, cap) : dp;
-    const double lm = dm < 0.0 ? fmax(dm, -cap) : dm;
+    const double lp = (dp > 0.0 && cap < dp) ? cap : dp;      // d+ > 0 ? min(d+, 2b) : d+
+    const double lm = (dm < 0.0 && dm < -cap) ? -cap : dm;    // d- < 0 ? max(d-, -2b) : d-
     return sf * ((b + c1 * lp) + c2 * lm);
 }
 
@@ -144,19 +145,64 @@ __device__ __forceinline__ double pencil_courant(const MarchArgs &p, long long o
     }
 }
 
+// ---------------------------------------------------------------- block reduction helper
+template <int NV>
+__device__ __forceinline__ void block_reduce_sum(double (&val)[NV], double *smem /* [NV][32] */)
+{
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int nw = (blockDim.x + 31) >> 5;
+#pragma unroll
+    for (int k = 0; k < NV; ++k) {
+        double x = val[k];
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) x += __shfl_down_sync(0xffffffffu, x, off);
+        if (lane == 0) smem[k * 32 + wid] = x;
+    }
+    __syncthreads();
+    if (wid == 0) {
+#pragma unroll
+        for (int k = 0; k < NV; ++k) {
+            double x = lane < nw ? smem[k * 32 + lane] : 0.0;
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) x += __shfl_down_sync(0xffffffffu, x, off);
+            val[k] = x;
+        }
+    }
+}
+
 // ---------------------------------------------------------------- march kernel
 // In-place remap with |s| < 1 (k = 0). Window (g_{i-1}, g_i, g_{i+1}, g_{i+2}) in registers;
 // buf/nxt hold the next 2U loads so that U independent loads per thread are always in flight.
-template <int VEC, int U, int KIND, int BC>
+template <int VEC, int U, int KIND, int BC, bool MOM>
 __global__ void __launch_bounds__(256)
 march_kernel(const MarchArgs p)
 {
     typedef V<VEC> T;
+    __shared__ double red[MOM ? 10 * 32 : 1];
     const long long innerV = p.inner / VEC;
-    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= p.outer * innerV) return;
-    const long long o = t / innerV;
-    const long long e0 = (t - o * innerV) * VEC;
+    long long o, ev;
+    bool active;
+    if (MOM) {
+        // CTA-tiled: blockIdx.x = o * tiles + tile, a CTA never straddles spatial cells
+        o = blockIdx.x / p.tiles;
+        const int tile = blockIdx.x - (int)o * p.tiles;
+        const int lt = threadIdx.x;
+        ev = (long long)tile * p.per_tile + lt;
+        active = lt < p.per_tile && ev < innerV;
+    } else {
+        const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+        active = t < p.outer * innerV;
+        o = t / innerV;
+        ev = t - o * innerV;
+        if (!active) return;
+    }
+    double mom[10];
+    if (MOM) {
+#pragma unroll
+        for (int k = 0; k < 10; ++k) mom[k] = 0.0;
+    }
+    if (active) {
+    const long long e0 = ev * VEC;
     const int n = p.n;
     const long long stride = p.inner;
     double *base = p.f + (o * n) * stride + e0;
@@ -206,6 +252,9 @@ march_kernel(const MarchArgs p)
         }
     }
     T a1 = gm1;                                  // g_{i-1}
+    double s0[VEC], s1[VEC], s2[VEC];            // sum f, sum vz f, sum vz^2 f along the march (MOM)
+#pragma unroll
+    for (int l = 0; l < VEC; ++l) { s0[l] = 0.0; s1[l] = 0.0; s2[l] = 0.0; }
 
     for (int i0 = 0; i0 < n; i0 += U) {
 #pragma unroll
@@ -226,12 +275,59 @@ march_kernel(const MarchArgs p)
                     phiprev.v[l] = phi;
                 }
                 stv<VEC>(base + (long long)i * stride, out);
+                if (MOM) {
+                    const double vz = vcentre(p.g, 2, i);
+#pragma unroll
+                    for (int l = 0; l < VEC; ++l) {
+                        const double tz = vz * out.v[l];
+                        s0[l] += out.v[l]; s1[l] += tz; s2[l] = fma(vz, tz, s2[l]);
+                    }
+                }
                 a1 = c0; c0 = c1v; c1v = c2v;
             }
         }
 #pragma unroll
         for (int u = 0; u < U; ++u) buf[u] = nxt[u];
     }
+    if (MOM) {
+        // thread's pencils sit at (jy, jx) = divmod(e0 + l, nvx): combine with vx, vy
+#pragma unroll
+        for (int l = 0; l < VEC; ++l) {
+            const long long e = e0 + l;
+            const int jy = (int)(e / p.g.nv[0]), jx = (int)(e - (long long)jy * p.g.nv[0]);
+            const double vx = vcentre(p.g, 0, jx), vy = vcentre(p.g, 1, jy);
+            const double x0 = vx * s0[l], y0 = vy * s0[l];
+            mom[0] += s0[l];
+            mom[1] += x0; mom[2] += y0; mom[3] += s1[l];
+            mom[4] = fma(vx, x0, mom[4]); mom[5] = fma(vx, y0, mom[5]); mom[6] = fma(vx, s1[l], mom[6]);
+            mom[7] = fma(vy, y0, mom[7]); mom[8] = fma(vy, s1[l], mom[8]); mom[9] += s2[l];
+        }
+    }
+    }   // active
+    if (MOM) {
+        block_reduce_sum<10>(mom, red);
+        if (threadIdx.x == 0) {
+#pragma unroll
+            for (int k = 0; k < 10; ++k) p.mom[(long long)blockIdx.x * 10 + k] = mom[k];
+        }
+    }
+}
+
+// Sums the per-CTA partial moments of the fused V_vz kernel in fixed order and scales by dV.
+__global__ void __launch_bounds__(256)
+mom_finalize_kernel(const double *__restrict__ part, int tiles, long long ns, double dV,
+                    double *__restrict__ n, double *__restrict__ j, double *__restrict__ P)
+{
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= ns * 10) return;
+    const long long cell = t / 10;
+    const int k = (int)(t - cell * 10);
+    double acc = 0.0;
+    for (int tl = 0; tl < tiles; ++tl) acc += part[(cell * tiles + tl) * 10 + k];
+    acc *= dV;
+    if (k == 0) n[cell] = acc;
+    else if (k < 4) j[(k - 1) * ns + cell] = acc;
+    else P[(k - 4) * ns + cell] = acc;
 }
 
 // ---------------------------------------------------------------- vx kernel (contiguous axis)
@@ -311,6 +407,214 @@ vx_kernel(const VxArgs p)
     }
 }
 
+// ---------------------------------------------------------------- fused V_vx + V_vy plane kernel
+// One (spatial cell, jvz) plane of nvy x nvx doubles is contiguous in memory (12.8 KB at 40^2).
+// Persistent CTAs loop over planes. A plane is brought into shared memory by ONE bulk async
+// copy (cp.async.bulk, TMA engine, completion on an mbarrier), NS planes in flight per CTA, so
+// no registers are tied up by loads in flight. The vx remap reads the plane from smem and
+// writes the result to a second smem buffer; the vy remap reads that buffer and stores straight
+// to global memory (in place: the input plane already sits in smem). f is read once and
+// written once for both sweeps.
+//   vx items: (row r, column pair q): 3 face fluxes for 2 cells;   smem address = 16 * item
+//   vy items: (row pair rp, column pair q): 3 face fluxes x 2 columns for 4 cells
+// Courant numbers are per row (vx) / per column (vy); they are computed once per plane into
+// smem by the first nvy + nvx threads (double-buffered by plane parity).
+struct PlaneArgs {
+    double *f;
+    long long planes;       // ns * nvz
+    int nvx, nvy, nvz;
+    int hx, hy;             // nvx / 2, nvy / 2
+    float inv_hx;           // 1 / hx for the item -> (row, pair) split
+    double dt;
+    const double *E, *B;
+    GridDev g;
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n" : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void bulk_load(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+__device__ __forceinline__ void split_item(int item, int h, float inv_h, int &r, int &q)
+{
+    r = __float2int_rd(((float)item + 0.5f) * inv_h);
+    q = item - r * h;
+}
+
+// Courant triple from a signed Courant number, with the polynomial constants by multiplication
+__device__ __forceinline__ void courant3(double s, double &sf, double &c1, double &c2)
+{
+    const double fr = fabs(s);
+    const double om = 1.0 - fr;
+    sf = s;
+    c1 = (om * (2.0 - fr)) * (1.0 / 6.0);
+    c2 = (om * (1.0 + fr)) * (1.0 / 6.0);
+}
+
+template <int NS>
+__global__ void __launch_bounds__(448, 2)
+vxy_kernel(const PlaneArgs p)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int T = blockDim.x;
+    const int tid = threadIdx.x;
+    const int nvx = p.nvx, nvy = p.nvy, hx = p.hx, hy = p.hy;
+    const int cells = nvx * nvy;
+    const uint32_t plane_bytes = (uint32_t)cells * 8u;
+    double *inbuf = reinterpret_cast<double *>(smem_raw);                 // [NS][cells]
+    double *xbuf = inbuf + (size_t)NS * cells;                           // [cells]
+    double *cx = xbuf + cells;                                           // [2][3][nvy]  row Courant triples
+    double *cy = cx + 6 * nvy;                                           // [2][3][nvx]  column Courant triples
+    uint64_t *bars = reinterpret_cast<uint64_t *>(cy + 6 * nvx);         // [NS]
+
+    if (tid == 0) {
+        for (int s = 0; s < NS; ++s) mbar_init(&bars[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+
+    const long long first = blockIdx.x;
+    const long long step = gridDim.x;
+    const long long K = first < p.planes ? (p.planes - first + step - 1) / step : 0;
+
+    if (tid == 0) {
+        for (int k = 0; k < NS - 1 && k < K; ++k) {
+            mbar_expect_tx(&bars[k], plane_bytes);
+            bulk_load(inbuf + (size_t)k * cells, p.f + (first + k * step) * cells, plane_bytes, &bars[k]);
+        }
+    }
+
+    const double dtdvx = p.dt / p.g.dv[0];
+    const double dtdvy = p.dt / p.g.dv[1];
+
+    for (long long k = 0; k < K; ++k) {
+        const long long plane = first + k * step;
+        const int slot = (int)(k % NS);
+        const uint32_t parity = (uint32_t)((k / NS) & 1);
+        const int par = (int)(k & 1);
+        double *cxp = cx + par * 3 * nvy;
+        double *cyp = cy + par * 3 * nvx;
+
+        // prefetch plane k+NS-1 into the slot consumed in iteration k-1 (all threads passed S2 of k-1)
+        if (tid == 0 && k + NS - 1 < K) {
+            const int ns_slot = (int)((k + NS - 1) % NS);
+            mbar_expect_tx(&bars[ns_slot], plane_bytes);
+            bulk_load(inbuf + (size_t)ns_slot * cells, p.f + (plane + (NS - 1) * step) * cells, plane_bytes, &bars[ns_slot]);
+        }
+
+        // Courant numbers of this plane: rows (a_x needs vy, vz) and columns (a_y needs vz, vx)
+        {
+            const long long cell = plane / p.nvz;
+            const int jz = (int)(plane - cell * p.nvz);
+            if (tid < nvy) {
+                const double a = accel_at(p.g, p.E, p.B, 0, cell, vcentre(p.g, 1, tid), vcentre(p.g, 2, jz));
+                double sf, c1, c2;
+                courant3(a * dtdvx, sf, c1, c2);
+                cxp[tid] = sf; cxp[nvy + tid] = c1; cxp[2 * nvy + tid] = c2;
+            } else if (tid >= T - nvx) {
+                const int jx = tid - (T - nvx);
+                const double a = accel_at(p.g, p.E, p.B, 1, cell, vcentre(p.g, 2, jz), vcentre(p.g, 0, jx));
+                double sf, c1, c2;
+                courant3(a * dtdvy, sf, c1, c2);
+                cyp[jx] = sf; cyp[nvx + jx] = c1; cyp[2 * nvx + jx] = c2;
+            }
+        }
+        mbar_wait(&bars[slot], parity);
+        __syncthreads();                         // S1: Courant numbers visible; xbuf free (vy of k-1 done)
+
+        // ---- vx remap: inbuf[slot] -> xbuf
+        const double2 *in2 = reinterpret_cast<const double2 *>(inbuf + (size_t)slot * cells);
+        double2 *xb2 = reinterpret_cast<double2 *>(xbuf);
+        for (int item = tid; item < nvy * hx; item += T) {
+            int r, q;
+            split_item(item, hx, p.inv_hx, r, q);
+            const double2 own = in2[item];
+            double2 lft = make_double2(0.0, 0.0), rgt = make_double2(0.0, 0.0);
+            if (q > 0) lft = in2[item - 1];
+            if (q < hx - 1) rgt = in2[item + 1];
+            const double sf = cxp[r], c1 = cxp[nvy + r], c2 = cxp[2 * nvy + r];
+            double ph0, ph1, ph2;
+            if (sf >= 0.0) {
+                ph0 = face_flux(lft.x, lft.y, own.x, sf, c1, c2);
+                ph1 = face_flux(lft.y, own.x, own.y, sf, c1, c2);
+                ph2 = face_flux(own.x, own.y, rgt.x, sf, c1, c2);
+            } else {
+                ph0 = face_flux(own.y, own.x, lft.y, sf, c1, c2);
+                ph1 = face_flux(rgt.x, own.y, own.x, sf, c1, c2);
+                ph2 = face_flux(rgt.y, rgt.x, own.y, sf, c1, c2);
+            }
+            if (q == 0) ph0 = 0.0;               // closed velocity box (R7)
+            if (q == hx - 1) ph2 = 0.0;
+            xb2[item] = make_double2(own.x + (ph0 - ph1), own.y + (ph1 - ph2));
+        }
+        __syncthreads();                         // S2: xbuf complete; inbuf[slot] free for the next bulk load
+
+        // ---- vy remap: xbuf -> global (rows 2rp, 2rp+1 of column pair q)
+        double2 *out2 = reinterpret_cast<double2 *>(p.f + plane * cells);
+        for (int item = tid; item < hy * hx; item += T) {
+            int rp, q;
+            split_item(item, hx, p.inv_hx, rp, q);
+            const int r0 = 2 * rp;
+            double2 w[6];
+#pragma unroll
+            for (int j = 0; j < 6; ++j) {
+                const int r = r0 - 2 + j;
+                w[j] = (r >= 0 && r < nvy) ? xb2[r * hx + q] : make_double2(0.0, 0.0);
+            }
+            const double2 sf = *reinterpret_cast<const double2 *>(cyp + 2 * q);
+            const double2 c1 = *reinterpret_cast<const double2 *>(cyp + nvx + 2 * q);
+            const double2 c2 = *reinterpret_cast<const double2 *>(cyp + 2 * nvx + 2 * q);
+            double a0, a1, a2, b0, b1, b2;
+            if (sf.x >= 0.0) {
+                a0 = face_flux(w[0].x, w[1].x, w[2].x, sf.x, c1.x, c2.x);
+                a1 = face_flux(w[1].x, w[2].x, w[3].x, sf.x, c1.x, c2.x);
+                a2 = face_flux(w[2].x, w[3].x, w[4].x, sf.x, c1.x, c2.x);
+            } else {
+                a0 = face_flux(w[3].x, w[2].x, w[1].x, sf.x, c1.x, c2.x);
+                a1 = face_flux(w[4].x, w[3].x, w[2].x, sf.x, c1.x, c2.x);
+                a2 = face_flux(w[5].x, w[4].x, w[3].x, sf.x, c1.x, c2.x);
+            }
+            if (sf.y >= 0.0) {
+                b0 = face_flux(w[0].y, w[1].y, w[2].y, sf.y, c1.y, c2.y);
+                b1 = face_flux(w[1].y, w[2].y, w[3].y, sf.y, c1.y, c2.y);
+                b2 = face_flux(w[2].y, w[3].y, w[4].y, sf.y, c1.y, c2.y);
+            } else {
+                b0 = face_flux(w[3].y, w[2].y, w[1].y, sf.y, c1.y, c2.y);
+                b1 = face_flux(w[4].y, w[3].y, w[2].y, sf.y, c1.y, c2.y);
+                b2 = face_flux(w[5].y, w[4].y, w[3].y, sf.y, c1.y, c2.y);
+            }
+            if (rp == 0) { a0 = 0.0; b0 = 0.0; }
+            if (rp == hy - 1) { a2 = 0.0; b2 = 0.0; }
+            out2[r0 * hx + q] = make_double2(w[2].x + (a0 - a1), w[2].y + (b0 - b1));
+            out2[(r0 + 1) * hx + q] = make_double2(w[3].x + (a1 - a2), w[3].y + (b1 - b2));
+        }
+    }
+}
+
 // ---------------------------------------------------------------- shift kernel (slow path)
 // Periodic axis, any s: g_i = f_{i-k}, k = trunc(s), then the fractional remap with
 // sf = s - k. Out of place (src -> dst), one thread per pencil, modular indexing.
@@ -343,31 +647,6 @@ shift_kernel(const MarchArgs p, const double *__restrict__ src, double *__restri
         const double phi = flux(i);
         db[(long long)i * stride] = g(i) + (phiprev - phi);
         phiprev = phi;
-    }
-}
-
-// ---------------------------------------------------------------- block reduction helper
-template <int NV>
-__device__ __forceinline__ void block_reduce_sum(double (&val)[NV], double *smem /* [NV][32] */)
-{
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const int nw = (blockDim.x + 31) >> 5;
-#pragma unroll
-    for (int k = 0; k < NV; ++k) {
-        double x = val[k];
-#pragma unroll
-        for (int off = 16; off > 0; off >>= 1) x += __shfl_down_sync(0xffffffffu, x, off);
-        if (lane == 0) smem[k * 32 + wid] = x;
-    }
-    __syncthreads();
-    if (wid == 0) {
-#pragma unroll
-        for (int k = 0; k < NV; ++k) {
-            double x = lane < nw ? smem[k * 32 + lane] : 0.0;
-#pragma unroll
-            for (int off = 16; off > 0; off >>= 1) x += __shfl_down_sync(0xffffffffu, x, off);
-            val[k] = x;
-        }
     }
 }
 
