@@ -39,7 +39,8 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs index (default 3, headline)")
     ap.add_argument("--impl", default="mphv", choices=["mphv", "reference"])
-    ap.add_argument("--no-fusion", action="store_true", help="one kernel per sweep (for profiling)")
+    ap.add_argument("--fusion", type=int, default=2, choices=[0, 1, 2],
+                    help="mphv_set_fusion level: 0 one kernel per sweep, 1 pairwise fused, 2 whole V stage fused (default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -203,7 +204,7 @@ def run_mphv(args, w):
     peak_gbs, peak_src = (float(peaks["hbm_gbs"]), "measured") if "hbm_gbs" in peaks else (6650.0, "fallback")
 
     sim = mphv.Vlasov.from_workload(wr, device=dev)
-    sim.set_fusion(not args.no_fusion)
+    sim.set_fusion(args.fusion)
     f = torch.from_numpy(f0).to(dev)
     sim.bind_f(f)
     sim.set_fields(torch.from_numpy(E).to(dev), torch.from_numpy(B).to(dev))
@@ -273,7 +274,7 @@ def run_mphv(args, w):
         "config": {"workload": w.name, "cells_per_gpu": w.n_cells, "bytes_per_copy_of_f": w.n_cells * 8,
                    "step": "S_x,S_y[,S_z],V_vx,V_vy,V_vz + moments n,j,P every step",
                    "l2": "inputs larger than L2 (f is %.2f GB >> 126 MB); no flush needed" % (w.n_cells * 8 / 1e9),
-                   "fusion": not args.no_fusion, "parallelism": f"{world} independent problems" if world > 1 else "1 GPU"},
+                   "fusion": args.fusion, "parallelism": f"{world} independent problems" if world > 1 else "1 GPU"},
         "clocks": clk.summary(), "gpu_launches": launches, "roofline": roofline,
     }
 

@@ -146,9 +146,12 @@ int mphv_timing_slots(void);
 int mphv_get_timing(mphv_ctx *ctx, int slot, char *name, size_t name_cap, double *total_ms,
                     uint64_t *launches, double *alg_bytes_per_launch);
 
-/* Tuning knob for experiments and tests: 0 = unfused kernels only (one kernel per sweep),
- * 1 = allow fused kernels (default). Results agree up to fp64 rounding either way. */
-int mphv_set_fusion(mphv_ctx *ctx, int enabled);
+/* Tuning knob for experiments and tests. level 0 = one kernel per sweep; 1 = pairwise fused
+ * kernels (V_vx+V_vy per velocity plane, V_vz+moments); 2 = the whole V stage (three sweeps
+ * and the moments) in one pass over f (default; falls back to level 1 / 0 kernels for grids
+ * the cube kernel does not cover: nvx, nvy not multiples of 4, fewer than 3 velocity
+ * dimensions). Results agree up to fp64 rounding at every level. */
+int mphv_set_fusion(mphv_ctx *ctx, int level);
 
 const char *mphv_strerror(int code);
 /* Last error text of this context, or of the last failed mphv_create when ctx is NULL.

@@ -3,6 +3,7 @@
 // mphv_kernels.cuh; there is no CPU fallback.
 #include "../../include/mphv.h"
 #include "mphv_kernels.cuh"
+#include "mphv_vcube.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -28,6 +29,7 @@ struct mphv_ctx {
     int mom_tiles, mom_per_tile, mom_block;   // CTA tiling of the fused V_vz + moments kernel
     int sm_count;
     int vxy_T, vxy_grid; size_t vxy_smem;     // fused V_vx + V_vy plane kernel launch shape (0 = unsupported)
+    int cube_T, cube_grid; size_t cube_smem;  // whole-V-stage cube kernel launch shape (0 = unsupported)
     uint64_t launches;
     int fusion;
     int timing;
@@ -40,10 +42,11 @@ struct mphv_ctx {
 };
 
 enum { SLOT_SX0 = 0, SLOT_SX1, SLOT_SX2, SLOT_VX, SLOT_VY, SLOT_VZ, SLOT_MOM, SLOT_VXY, SLOT_VZMOM,
-       SLOT_SHIFT, SLOT_SUM, SLOT_AMAX, SLOT_COUNT };
+       SLOT_SHIFT, SLOT_SUM, SLOT_AMAX, SLOT_VCUBE, SLOT_VCUBE_MOM, SLOT_COUNT };
 static const char *const SLOT_NAMES[SLOT_COUNT] = {
     "sweep_x0", "sweep_x1", "sweep_x2", "sweep_vx", "sweep_vy", "sweep_vz", "moments",
-    "fused_vx_vy", "fused_vz_moments", "shift_periodic", "sum_f", "amax_fields" };
+    "fused_vx_vy", "fused_vz_moments", "shift_periodic", "sum_f", "amax_fields",
+    "fused_vx_vy_vz", "fused_vx_vy_vz_moments" };
 
 namespace {
 
@@ -191,6 +194,30 @@ int launch_vxy(mphv_ctx *c, double dt)
     return after_launch(c, "vxy_kernel");
 }
 
+const int CUBE_NS = 4;                  // planes in flight per CTA (TMA ring depth)
+
+// V_vx, V_vy, V_vz (+ moments if n != NULL) in one pass over f
+int launch_vcube(mphv_ctx *c, double dt, double *n, double *j, double *P)
+{
+    CubeArgs a;
+    std::memset(&a, 0, sizeof a);
+    a.f = c->f;
+    a.ns = (long long)c->ns;
+    a.nvx = c->grid.nv[0]; a.nvy = c->grid.nv[1]; a.nvz = c->grid.nv[2];
+    a.qx = a.nvx / 4;
+    a.items = a.nvy * a.qx;
+    a.dt = dt;
+    a.E = c->E; a.B = c->B;
+    a.n = n; a.j = j; a.P = P;
+    a.dV = c->dv[0] * c->dv[1] * c->dv[2];
+    a.g = c->gd;
+    const long long grid = (long long)c->ns < c->cube_grid ? (long long)c->ns : c->cube_grid;
+    Timed tm(c, n ? SLOT_VCUBE_MOM : SLOT_VCUBE, (n ? 56.0 : 48.0) * (double)c->nf);
+    if (n) vcube_kernel<CUBE_NS, true><<<(unsigned)grid, c->cube_T, c->cube_smem, c->stream>>>(a);
+    else   vcube_kernel<CUBE_NS, false><<<(unsigned)grid, c->cube_T, c->cube_smem, c->stream>>>(a);
+    return after_launch(c, "vcube_kernel");
+}
+
 MarchArgs march_args_space(const mphv_ctx *c, int d, double dt)
 {
     MarchArgs a;
@@ -277,6 +304,7 @@ int do_v_stage(mphv_ctx *c, double dt, double *n, double *j, double *P)
 {
     int st;
     const bool ax = c->grid.nv[0] > 1, ay = c->grid.nv[1] > 1, az = c->grid.nv[2] > 1;
+    if (c->fusion >= 2 && c->cube_T > 0) return launch_vcube(c, dt, n, j, P);
     if (c->fusion && ax && ay && c->vxy_T > 0) {
         if ((st = launch_vxy(c, dt)) != MPHV_OK) return st;
     } else {
@@ -369,7 +397,7 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
     c->ns = (size_t)grid->nx[0] * grid->nx[1] * grid->nx[2];
     c->nvel = (size_t)grid->nv[0] * grid->nv[1] * grid->nv[2];
     c->nf = c->ns * c->nvel;
-    c->fusion = 1;
+    c->fusion = 2;
     for (int d = 0; d < 3; ++d) {
         c->dx[d] = grid->nx[d] > 1 ? (box->xhi[d] - box->xlo[d]) / (double)grid->nx[d] : 1.0;
         c->dv[d] = grid->nv[d] > 1 ? (box->vhi[d] - box->vlo[d]) / (double)grid->nv[d] : 1.0;
@@ -404,6 +432,24 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
             int per_sm = 0;
             if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, vxy_kernel<3>, T, smem) == cudaSuccess && per_sm > 0) {
                 c->vxy_T = T; c->vxy_smem = smem; c->vxy_grid = per_sm * c->sm_count;
+            }
+        }
+        cudaGetLastError();
+    }
+    c->cube_T = 0;
+    if (grid->nv[0] % 4 == 0 && grid->nv[1] % 4 == 0 && grid->nv[2] >= 4) {
+        const int nvx = grid->nv[0], nvy = grid->nv[1], nvz = grid->nv[2];
+        const int items = nvy * (nvx / 4);
+        const int T = (items + 31) / 32 * 32;
+        const size_t smem = ((size_t)(CUBE_NS + 2) * nvx * nvy + 9 * (size_t)(nvx + nvy) + (nvz + 2) + 12 + 320 + CUBE_NS) * sizeof(double);
+        int max_optin = 0;
+        cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+        if (T <= 512 && nvx + nvy <= T && nvz + 2 <= T && smem <= (size_t)max_optin &&
+            cudaFuncSetAttribute(vcube_kernel<CUBE_NS, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess &&
+            cudaFuncSetAttribute(vcube_kernel<CUBE_NS, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess) {
+            int per_sm = 0;
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, vcube_kernel<CUBE_NS, true>, T, smem) == cudaSuccess && per_sm > 0) {
+                c->cube_T = T; c->cube_smem = smem; c->cube_grid = per_sm * c->sm_count;
             }
         }
         cudaGetLastError();
@@ -584,7 +630,7 @@ uint64_t mphv_launch_count(const mphv_ctx *c) { return c ? c->launches : 0; }
 int mphv_set_fusion(mphv_ctx *c, int enabled)
 {
     if (!c) return MPHV_ERR_ARG;
-    c->fusion = enabled ? 1 : 0;
+    c->fusion = enabled < 0 ? 0 : (enabled > 2 ? 2 : enabled);
     return MPHV_OK;
 }
 

@@ -175,8 +175,11 @@ def mphv_launch_count(ctx) -> int:
     return int(lib().mphv_launch_count(ctx))
 
 
-def mphv_set_fusion(ctx, enabled: bool):
-    _check(ctx, lib().mphv_set_fusion(ctx, 1 if enabled else 0))
+def mphv_set_fusion(ctx, level):
+    """level: 0 / 1 / 2 as in include/mphv.h; True means the default (2), False means 0."""
+    if isinstance(level, bool):
+        level = 2 if level else 0
+    _check(ctx, lib().mphv_set_fusion(ctx, int(level)))
 
 
 def mphv_set_timing(ctx, enabled: bool):
@@ -288,8 +291,8 @@ class Vlasov:
     def launches(self) -> int:
         return mphv_launch_count(self.ctx)
 
-    def set_fusion(self, enabled: bool):
-        mphv_set_fusion(self.ctx, enabled)
+    def set_fusion(self, level):
+        mphv_set_fusion(self.ctx, level)
 
     def set_timing(self, enabled: bool):
         mphv_set_timing(self.ctx, enabled)

@@ -97,7 +97,7 @@ def test_each_sweep_matches_oracle(torch_cuda, mphv, orc, nx, nv, bc, sign):
 
 @pytest.mark.parametrize("nx,nv,bc", SHAPES + [((4, 4, 1), (40, 40, 8), (0, 1, 0)), ((4, 4, 1), (20, 36, 4), (0, 0, 0)),
                                             ((4, 4, 1), (4, 4, 4), (0, 1, 0)), ((4, 4, 1), (64, 8, 1), (0, 1, 0))])
-@pytest.mark.parametrize("fusion", [False, True])
+@pytest.mark.parametrize("fusion", [0, 1, 2])
 def test_full_step_and_moments_fused_and_unfused(torch_cuda, mphv, orc, nx, nv, bc, fusion):
     """mphv_step_moments (fused plane kernel vx+vy, fused vz+moments when fusion is on) against
     oracle step + oracle moments, ragged and odd shapes included (odd extents fall back to the
@@ -153,7 +153,7 @@ def test_limiter_active_data_matches_oracle(torch_cuda, mphv, orc):
     assert rel_err(g, p.f_ref, AX_V[2]) <= TOL_SWEEP
 
 
-@pytest.mark.parametrize("fusion", [False, True])
+@pytest.mark.parametrize("fusion", [0, 1, 2])
 def test_config0_landau_20_steps_and_moments(torch_cuda, mphv, orc, fusion):
     from paper_2305_01487_b200 import inputs
     w = inputs.config(0)
@@ -187,7 +187,7 @@ def check_moments(p, orc, g):
             k += 1
 
 
-@pytest.mark.parametrize("fusion", [False, True])
+@pytest.mark.parametrize("fusion", [0, 1, 2])
 def test_config1_harris_steps_and_moments(torch_cuda, mphv, orc, fusion):
     from paper_2305_01487_b200 import inputs
     w = inputs.config(1)
