@@ -29,7 +29,7 @@ struct mphv_ctx {
     int mom_tiles, mom_per_tile, mom_block;   // CTA tiling of the fused V_vz + moments kernel
     int sm_count;
     int vxy_T, vxy_grid; size_t vxy_smem;     // fused V_vx + V_vy plane kernel launch shape (0 = unsupported)
-    int cube_T, cube_grid; size_t cube_smem;  // whole-V-stage cube kernel launch shape (0 = unsupported)
+    int cube_T, cube_grid, cube_variant; size_t cube_smem;  // whole-V-stage cube kernel launch shape (T = 0: unsupported)
     uint64_t launches;
     int fusion;
     int timing;
@@ -196,6 +196,26 @@ int launch_vxy(mphv_ctx *c, double dt)
 
 const int CUBE_NS = 4;                  // planes in flight per CTA (TMA ring depth)
 
+// The cube kernel is specialised for the velocity-plane shapes of the BASELINE.json configs
+// (40x40, 32x32: compile-time row strides) and has a generic instance for everything else.
+enum { CUBE_40 = 0, CUBE_32 = 1, CUBE_GEN = 2 };
+
+template <bool MOM> void *cube_fn(int variant)
+{
+    switch (variant) {
+    case CUBE_40: return (void *)vcube_kernel<CUBE_NS, MOM, 40, 40, 416, 1>;
+    case CUBE_32: return (void *)vcube_kernel<CUBE_NS, MOM, 32, 32, 256, 2>;
+    default:      return (void *)vcube_kernel<CUBE_NS, MOM, 0, 0, 512, 1>;
+    }
+}
+
+size_t cube_smem_bytes(int nvx, int nvy, int nvz)
+{
+    const size_t cells = (size_t)nvx * nvy, xcells = (size_t)nvx * (nvy + 4);
+    return (CUBE_NS * cells + CUBE_NXB * xcells + CUBE_NT * 4 * (size_t)(nvx + nvy) + nvz + 6 * CUBE_FLD + 320) * sizeof(double)
+           + (CUBE_NS + 2) * sizeof(uint64_t);
+}
+
 // V_vx, V_vy, V_vz (+ moments if n != NULL) in one pass over f
 int launch_vcube(mphv_ctx *c, double dt, double *n, double *j, double *P)
 {
@@ -204,17 +224,16 @@ int launch_vcube(mphv_ctx *c, double dt, double *n, double *j, double *P)
     a.f = c->f;
     a.ns = (long long)c->ns;
     a.nvx = c->grid.nv[0]; a.nvy = c->grid.nv[1]; a.nvz = c->grid.nv[2];
-    a.qx = a.nvx / 4;
-    a.items = a.nvy * a.qx;
     a.dt = dt;
     a.E = c->E; a.B = c->B;
     a.n = n; a.j = j; a.P = P;
     a.dV = c->dv[0] * c->dv[1] * c->dv[2];
     a.g = c->gd;
-    const long long grid = (long long)c->ns < c->cube_grid ? (long long)c->ns : c->cube_grid;
     Timed tm(c, n ? SLOT_VCUBE_MOM : SLOT_VCUBE, (n ? 56.0 : 48.0) * (double)c->nf);
-    if (n) vcube_kernel<CUBE_NS, true><<<(unsigned)grid, c->cube_T, c->cube_smem, c->stream>>>(a);
-    else   vcube_kernel<CUBE_NS, false><<<(unsigned)grid, c->cube_T, c->cube_smem, c->stream>>>(a);
+    void *fn = n ? cube_fn<true>(c->cube_variant) : cube_fn<false>(c->cube_variant);
+    void *args[] = { &a };
+    cudaError_t e = cudaLaunchKernel(fn, dim3((unsigned)c->cube_grid), dim3((unsigned)c->cube_T), args, c->cube_smem, c->stream);
+    if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(c, e, "vcube_kernel launch"); }
     return after_launch(c, "vcube_kernel");
 }
 
@@ -441,15 +460,20 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
         const int nvx = grid->nv[0], nvy = grid->nv[1], nvz = grid->nv[2];
         const int items = nvy * (nvx / 4);
         const int T = (items + 31) / 32 * 32;
-        const size_t smem = ((size_t)(CUBE_NS + 2) * nvx * nvy + 9 * (size_t)(nvx + nvy) + (nvz + 2) + 12 + 320 + CUBE_NS) * sizeof(double);
+        const int variant = (nvx == 40 && nvy == 40) ? CUBE_40 : (nvx == 32 && nvy == 32) ? CUBE_32 : CUBE_GEN;
+        const size_t smem = cube_smem_bytes(nvx, nvy, nvz);
         int max_optin = 0;
         cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-        if (T <= 512 && nvx + nvy <= T && nvz + 2 <= T && smem <= (size_t)max_optin &&
-            cudaFuncSetAttribute(vcube_kernel<CUBE_NS, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess &&
-            cudaFuncSetAttribute(vcube_kernel<CUBE_NS, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess) {
+        if (T <= 512 && nvx + nvy <= T && smem <= (size_t)max_optin &&
+            cudaFuncSetAttribute(cube_fn<true>(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess &&
+            cudaFuncSetAttribute(cube_fn<false>(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess) {
             int per_sm = 0;
-            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, vcube_kernel<CUBE_NS, true>, T, smem) == cudaSuccess && per_sm > 0) {
-                c->cube_T = T; c->cube_smem = smem; c->cube_grid = per_sm * c->sm_count;
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, cube_fn<true>(variant), T, smem) == cudaSuccess && per_sm > 0) {
+                long long g = (long long)per_sm * c->sm_count;
+                const long long gmin = ((long long)c->ns + CUBE_FLD - 1) / CUBE_FLD;   // <= CUBE_FLD cells per CTA
+                if (g < gmin) g = ((gmin + c->sm_count - 1) / c->sm_count) * c->sm_count;
+                if (g > (long long)c->ns) g = (long long)c->ns;
+                c->cube_T = T; c->cube_smem = smem; c->cube_grid = (int)g; c->cube_variant = variant;
             }
         }
         cudaGetLastError();
