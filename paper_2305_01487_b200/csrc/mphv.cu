@@ -4,6 +4,7 @@
 #include "../../include/mphv.h"
 #include "mphv_kernels.cuh"
 #include "mphv_vcube.cuh"
+#include "mphv_march.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -146,10 +147,10 @@ int launch_march(mphv_ctx *c, const MarchArgs &a)
     Timed tm(c, KIND == KIND_SPACE ? SLOT_SX0 + a.dim : SLOT_VX + a.dim, 16.0 * (double)c->nf);
     if (a.inner % 2 == 0) {
         const long long threads = a.outer * (a.inner / 2);
-        march_kernel<2, 4, KIND, BC, false><<<grid_for(threads, block), block, 0, c->stream>>>(a);
+        march2_kernel<2, 4, KIND, BC, false, 2><<<grid_for(threads, block), block, 0, c->stream>>>(a);
     } else {
         const long long threads = a.outer * a.inner;
-        march_kernel<1, 4, KIND, BC, false><<<grid_for(threads, block), block, 0, c->stream>>>(a);
+        march2_kernel<1, 4, KIND, BC, false, 2><<<grid_for(threads, block), block, 0, c->stream>>>(a);
     }
     return after_launch(c, "march_kernel");
 }
@@ -168,8 +169,8 @@ int launch_vz_moments(mphv_ctx *c, MarchArgs a, double *n, double *j, double *P)
     a.per_tile = c->mom_per_tile;
     a.dV = c->dv[0] * c->dv[1] * c->dv[2];
     const unsigned grid = (unsigned)(c->ns * (size_t)c->mom_tiles);
-    if (a.inner % 2 == 0) march_kernel<2, 4, KIND_VEL, BC_WALL, true><<<grid, c->mom_block, 0, c->stream>>>(a);
-    else                  march_kernel<1, 4, KIND_VEL, BC_WALL, true><<<grid, c->mom_block, 0, c->stream>>>(a);
+    if (a.inner % 2 == 0) march2_kernel<2, 4, KIND_VEL, BC_WALL, true, 2><<<grid, c->mom_block, 0, c->stream>>>(a);
+    else                  march2_kernel<1, 4, KIND_VEL, BC_WALL, true, 2><<<grid, c->mom_block, 0, c->stream>>>(a);
     int st = after_launch(c, "march_kernel(vz+moments)");
     if (st != MPHV_OK) return st;
     mom_finalize_kernel<<<grid_for((long long)c->ns * 10, 256), 256, 0, c->stream>>>(a.mom, c->mom_tiles, (long long)c->ns, a.dV, n, j, P);
