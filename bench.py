@@ -39,8 +39,8 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs index (default 3, headline)")
     ap.add_argument("--impl", default="mphv", choices=["mphv", "reference"])
-    ap.add_argument("--fusion", type=int, default=2, choices=[0, 1, 2],
-                    help="mphv_set_fusion level: 0 one kernel per sweep, 1 pairwise fused, 2 whole V stage fused (default)")
+    ap.add_argument("--fusion", type=int, default=1, choices=[0, 1, 2],
+                    help="mphv_set_fusion level: 0 one kernel per sweep, 1 pairwise fused, 2 whole V stage in one kernel; default 1")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)

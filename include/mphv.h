@@ -147,10 +147,10 @@ int mphv_get_timing(mphv_ctx *ctx, int slot, char *name, size_t name_cap, double
                     uint64_t *launches, double *alg_bytes_per_launch);
 
 /* Tuning knob for experiments and tests. level 0 = one kernel per sweep; 1 = pairwise fused
- * kernels (V_vx+V_vy per velocity plane, V_vz+moments); 2 = the whole V stage (three sweeps
- * and the moments) in one pass over f (default; falls back to level 1 / 0 kernels for grids
- * the cube kernel does not cover: nvx, nvy not multiples of 4, fewer than 3 velocity
- * dimensions). Results agree up to fp64 rounding at every level. */
+ * kernels (V_vx+V_vy per velocity plane, V_vz+moments; the default, fastest measured on B200);
+ * 2 = the whole V stage (three sweeps and the moments) in one pass over f. Levels 1 and 2 fall
+ * back to lower-level kernels for grids their kernels do not cover (nvx, nvy not multiples of 4
+ * resp. 2, fewer than 3 velocity dimensions). Results agree up to fp64 rounding at every level. */
 int mphv_set_fusion(mphv_ctx *ctx, int level);
 
 const char *mphv_strerror(int code);

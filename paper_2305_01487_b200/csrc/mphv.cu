@@ -30,7 +30,7 @@ struct mphv_ctx {
     int mom_tiles, mom_per_tile, mom_block;   // CTA tiling of the fused V_vz + moments kernel
     int sm_count;
     int vxy_T, vxy_grid; size_t vxy_smem;     // fused V_vx + V_vy plane kernel launch shape (0 = unsupported)
-    int cube_T, cube_grid, cube_variant; size_t cube_smem;  // whole-V-stage cube kernel launch shape (T = 0: unsupported)
+    int cube_T, cube_grid, cube_variant, plane_grid; size_t cube_smem, plane_smem;  // whole-V-stage cube kernel launch shape (T = 0: unsupported)
     uint64_t launches;
     int fusion;
     int timing;
@@ -195,7 +195,8 @@ int launch_vxy(mphv_ctx *c, double dt)
     return after_launch(c, "vxy_kernel");
 }
 
-const int CUBE_NS = 4;                  // planes in flight per CTA (TMA ring depth)
+const int CUBE_NS = 4;                  // planes in flight per CTA (TMA ring depth), whole-V-stage kernel
+const int PLANE_NS = 3;                 // same for the V_vx + V_vy variant (two CTAs per SM)
 
 // The cube kernel is specialised for the velocity-plane shapes of the BASELINE.json configs
 // (40x40, 32x32: compile-time row strides) and has a generic instance for everything else.
@@ -204,21 +205,31 @@ enum { CUBE_40 = 0, CUBE_32 = 1, CUBE_GEN = 2 };
 template <bool MOM> void *cube_fn(int variant)
 {
     switch (variant) {
-    case CUBE_40: return (void *)vcube_kernel<CUBE_NS, MOM, 40, 40, 416, 1>;
-    case CUBE_32: return (void *)vcube_kernel<CUBE_NS, MOM, 32, 32, 256, 2>;
-    default:      return (void *)vcube_kernel<CUBE_NS, MOM, 0, 0, 512, 1>;
+    case CUBE_40: return (void *)vcube_kernel<CUBE_NS, true, MOM, 40, 40, 416, 1>;
+    case CUBE_32: return (void *)vcube_kernel<CUBE_NS, true, MOM, 32, 32, 256, 2>;
+    default:      return (void *)vcube_kernel<CUBE_NS, true, MOM, 0, 0, 512, 1>;
     }
 }
 
-size_t cube_smem_bytes(int nvx, int nvy, int nvz)
+// the same pipeline without the V_vz stage (V_vx + V_vy per plane)
+void *plane_fn(int variant)
 {
-    const size_t cells = (size_t)nvx * nvy, xcells = (size_t)nvx * (nvy + 4);
-    return (CUBE_NS * cells + CUBE_NXB * xcells + CUBE_NT * 4 * (size_t)(nvx + nvy) + nvz + 6 * CUBE_FLD + 320) * sizeof(double)
-           + (CUBE_NS + 2) * sizeof(uint64_t);
+    switch (variant) {
+    case CUBE_40: return (void *)vcube_kernel<PLANE_NS, false, false, 40, 40, 416, 2>;
+    case CUBE_32: return (void *)vcube_kernel<PLANE_NS, false, false, 32, 32, 256, 3>;
+    default:      return (void *)vcube_kernel<PLANE_NS, false, false, 0, 0, 512, 1>;
+    }
 }
 
-// V_vx, V_vy, V_vz (+ moments if n != NULL) in one pass over f
-int launch_vcube(mphv_ctx *c, double dt, double *n, double *j, double *P)
+size_t cube_smem_bytes(int nvx, int nvy, int nvz, int ns, bool reduce)
+{
+    const size_t cells = (size_t)nvx * nvy, xcells = (size_t)nvx * (nvy + 4);
+    return (ns * cells + CUBE_NXB * xcells + CUBE_NT * 4 * (size_t)(nvx + nvy) + nvz + 6 * CUBE_FLD + (reduce ? 320 : 0)) * sizeof(double)
+           + (ns + 2) * sizeof(uint64_t);
+}
+
+// V_vx, V_vy, V_vz (+ moments if n != NULL) in one pass over f; with_vz = false: V_vx, V_vy only
+int launch_vcube(mphv_ctx *c, double dt, bool with_vz, double *n, double *j, double *P)
 {
     CubeArgs a;
     std::memset(&a, 0, sizeof a);
@@ -230,10 +241,11 @@ int launch_vcube(mphv_ctx *c, double dt, double *n, double *j, double *P)
     a.n = n; a.j = j; a.P = P;
     a.dV = c->dv[0] * c->dv[1] * c->dv[2];
     a.g = c->gd;
-    Timed tm(c, n ? SLOT_VCUBE_MOM : SLOT_VCUBE, (n ? 56.0 : 48.0) * (double)c->nf);
-    void *fn = n ? cube_fn<true>(c->cube_variant) : cube_fn<false>(c->cube_variant);
+    Timed tm(c, !with_vz ? SLOT_VXY : n ? SLOT_VCUBE_MOM : SLOT_VCUBE, (!with_vz ? 32.0 : n ? 56.0 : 48.0) * (double)c->nf);
+    void *fn = !with_vz ? plane_fn(c->cube_variant) : n ? cube_fn<true>(c->cube_variant) : cube_fn<false>(c->cube_variant);
     void *args[] = { &a };
-    cudaError_t e = cudaLaunchKernel(fn, dim3((unsigned)c->cube_grid), dim3((unsigned)c->cube_T), args, c->cube_smem, c->stream);
+    cudaError_t e = cudaLaunchKernel(fn, dim3((unsigned)(with_vz ? c->cube_grid : c->plane_grid)), dim3((unsigned)c->cube_T), args,
+                                     with_vz ? c->cube_smem : c->plane_smem, c->stream);
     if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(c, e, "vcube_kernel launch"); }
     return after_launch(c, "vcube_kernel");
 }
@@ -324,8 +336,10 @@ int do_v_stage(mphv_ctx *c, double dt, double *n, double *j, double *P)
 {
     int st;
     const bool ax = c->grid.nv[0] > 1, ay = c->grid.nv[1] > 1, az = c->grid.nv[2] > 1;
-    if (c->fusion >= 2 && c->cube_T > 0) return launch_vcube(c, dt, n, j, P);
-    if (c->fusion && ax && ay && c->vxy_T > 0) {
+    if (c->fusion >= 2 && c->cube_T > 0) return launch_vcube(c, dt, true, n, j, P);
+    if (c->fusion && c->cube_T > 0 && c->plane_grid > 0) {
+        if ((st = launch_vcube(c, dt, false, nullptr, nullptr, nullptr)) != MPHV_OK) return st;
+    } else if (c->fusion && ax && ay && c->vxy_T > 0) {
         if ((st = launch_vxy(c, dt)) != MPHV_OK) return st;
     } else {
         if (ax && (st = do_sweep_v(c, 0, dt)) != MPHV_OK) return st;
@@ -417,7 +431,7 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
     c->ns = (size_t)grid->nx[0] * grid->nx[1] * grid->nx[2];
     c->nvel = (size_t)grid->nv[0] * grid->nv[1] * grid->nv[2];
     c->nf = c->ns * c->nvel;
-    c->fusion = 2;
+    c->fusion = 1;
     for (int d = 0; d < 3; ++d) {
         c->dx[d] = grid->nx[d] > 1 ? (box->xhi[d] - box->xlo[d]) / (double)grid->nx[d] : 1.0;
         c->dv[d] = grid->nv[d] > 1 ? (box->vhi[d] - box->vlo[d]) / (double)grid->nv[d] : 1.0;
@@ -462,7 +476,8 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
         const int items = nvy * (nvx / 4);
         const int T = (items + 31) / 32 * 32;
         const int variant = (nvx == 40 && nvy == 40) ? CUBE_40 : (nvx == 32 && nvy == 32) ? CUBE_32 : CUBE_GEN;
-        const size_t smem = cube_smem_bytes(nvx, nvy, nvz);
+        const size_t smem = cube_smem_bytes(nvx, nvy, nvz, CUBE_NS, true);
+        const size_t psmem = cube_smem_bytes(nvx, nvy, nvz, PLANE_NS, false);
         int max_optin = 0;
         cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
         if (T <= 512 && nvx + nvy <= T && smem <= (size_t)max_optin &&
@@ -475,6 +490,14 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
                 if (g < gmin) g = ((gmin + c->sm_count - 1) / c->sm_count) * c->sm_count;
                 if (g > (long long)c->ns) g = (long long)c->ns;
                 c->cube_T = T; c->cube_smem = smem; c->cube_grid = (int)g; c->cube_variant = variant;
+                c->plane_grid = 0;
+                if (cudaFuncSetAttribute(plane_fn(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)psmem) == cudaSuccess &&
+                    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, plane_fn(variant), T, psmem) == cudaSuccess && per_sm > 0) {
+                    long long pg = (long long)per_sm * c->sm_count;
+                    if (pg < gmin) pg = ((gmin + c->sm_count - 1) / c->sm_count) * c->sm_count;
+                    if (pg > (long long)c->ns) pg = (long long)c->ns;
+                    c->plane_grid = (int)pg; c->plane_smem = psmem;
+                }
             }
         }
         cudaGetLastError();

@@ -95,7 +95,9 @@ __device__ __forceinline__ void courant_entry(double a, double dtdv, double *dst
     dst[3] = 0.0;
 }
 
-template <int NS, bool MOM, int NVX, int NVY, int TMAX, int MINB>
+// VZ = false: V_vx and V_vy only (the V_vy result is stored straight to global memory; V_vz and the
+// moments are left to the march kernel) -- no per-thread march state, so two CTAs fit on an SM.
+template <int NS, bool VZ, bool MOM, int NVX, int NVY, int TMAX, int MINB>
 __global__ void __launch_bounds__(TMAX, MINB)
 vcube_kernel(const CubeArgs p)
 {
@@ -112,8 +114,8 @@ vcube_kernel(const CubeArgs p)
     double *taby = tabx + CUBE_NT * 4 * nvy;                            // [NT][nvx][4] column Courant data
     double *vzt = taby + CUBE_NT * 4 * nvx;                             // [nvz] vz centres
     double *fld = vzt + nvz;                                            // [CUBE_FLD][6] E, B of this CTA's cells
-    double *red = fld + 6 * CUBE_FLD;                                   // [10][32]
-    uint64_t *bars = reinterpret_cast<uint64_t *>(red + 320);           // [NS] TMA full, [2] xbar
+    double *red = fld + 6 * CUBE_FLD;                                   // [10][32] (VZ && MOM only)
+    uint64_t *bars = reinterpret_cast<uint64_t *>(red + (VZ && MOM ? 320 : 0));   // [NS] TMA full, [2] xbar
 
     const long long c_begin = (p.ns * (long long)blockIdx.x) / gridDim.x;
     const long long c_end = (p.ns * ((long long)blockIdx.x + 1)) / gridDim.x;
@@ -269,7 +271,7 @@ vcube_kernel(const CubeArgs p)
             if (++jzT == nvz) { jzT = 0; ++cellT; }
         }
         if (act) {
-            if (jzB == 0) {                          // new cube: V_vz Courant data of the 4 pencils
+            if (VZ && jzB == 0) {                    // new cube: V_vz Courant data of the 4 pencils
                 const double *fl = fld + 6 * cellB;
                 const double vx = vcentre(p.g, 0, jx);
 #pragma unroll
@@ -294,6 +296,11 @@ vcube_kernel(const CubeArgs p)
             const double2 t01 = *reinterpret_cast<const double2 *>(t);
             double nw[4];
             remap4(w, t01.x, t01.y, t[2], rq == 0, r0 + 4 == nvy, nw);
+            if (!VZ) {
+#pragma unroll
+                for (int m = 0; m < 4; ++m) outp[m * nvx] = nw[m];
+                outp += cells;
+            } else
             // window roles: !flip: ga = g_{j-1}, gb = g_j; flip: the other way round
             if (jzB == 0) {
 #pragma unroll
@@ -305,7 +312,7 @@ vcube_kernel(const CubeArgs p)
                 flip = !flip;
                 outp += cells;
             }
-            if (jzB == nvz - 1) {                    // drain: the two ghost planes behind the high wall are empty
+            if (VZ && jzB == nvz - 1) {              // drain: the two ghost planes behind the high wall are empty
                 const double zero[4] = { 0.0, 0.0, 0.0, 0.0 };
                 if (!flip) vz_step(M2(), ga, gb, zero, vzt[nvz - 1], outp); else vz_step(M2(), gb, ga, zero, vzt[nvz - 1], outp);
                 flip = !flip;
@@ -314,7 +321,7 @@ vcube_kernel(const CubeArgs p)
             }
         }
         if (jzB == nvz - 1) {
-            if (MOM) {
+            if (VZ && MOM) {
                 double mom[10];
 #pragma unroll
                 for (int i = 0; i < 10; ++i) mom[i] = 0.0;

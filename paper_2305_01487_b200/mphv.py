@@ -176,9 +176,9 @@ def mphv_launch_count(ctx) -> int:
 
 
 def mphv_set_fusion(ctx, level):
-    """level: 0 / 1 / 2 as in include/mphv.h; True means the default (2), False means 0."""
+    """level: 0 / 1 / 2 as in include/mphv.h; True means the default (1), False means 0."""
     if isinstance(level, bool):
-        level = 2 if level else 0
+        level = 1 if level else 0
     _check(ctx, lib().mphv_set_fusion(ctx, int(level)))
 
 
