@@ -7,8 +7,12 @@ A step = one pass of the whole hot path over the workload: the full split step S
 V_vx, V_vy, V_vz followed by the moments n, j, P (mphv_step_moments through the C ABI).
 Metric: phase-space cell-updates/s = cells x steps / time (BASELINE.json), fp64.
 N = 1 runs BASELINE.json configs[3] (2D3V 128x64x40^3, the headline roofline config).
-N > 1 (torchrun): every rank advances its own seeded copy of that workload (independent
-problems, no data-path collective), scaling = weak; time = max over ranks.
+N > 1 (torchrun): weak scaling by spatial block decomposition (the paper's own
+parallelisation): the periodic x axis is N times longer, every rank owns one
+configs[3]-sized block and exchanges its two boundary layers with both x neighbours before the
+S_x sweep (mphv_pack_halo -> NCCL send/recv -> mphv_sweep_x_halo); time = max over ranks.
+--decomp none instead runs N independent seeded problems (no exchange); --decomp halo at N = 1
+sends the spatial sweeps through the same pack / halo kernels with the block as its own neighbour.
 --impl reference times the CPU oracle (oracle/) on a bounded spatial sub-block of the same
 workload on the host cores; rank 0 only.
 """
@@ -41,6 +45,10 @@ def parse():
     ap.add_argument("--impl", default="mphv", choices=["mphv", "reference"])
     ap.add_argument("--fusion", type=int, default=1, choices=[0, 1, 2],
                     help="mphv_set_fusion level: 0 one kernel per sweep, 1 pairwise fused, 2 whole V stage in one kernel; default 1")
+    ap.add_argument("--decomp", default="auto", choices=["auto", "halo", "none"],
+                    help="'halo' = one spatially decomposed problem with neighbour exchange (the default for N > 1; "
+                         "at N = 1 the block is its own periodic neighbour), 'none' = N independent problems "
+                         "(the default at N = 1)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -193,9 +201,23 @@ def run_mphv(args, w):
     dev = torch.device("cuda", local)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
-    # each rank: its own seeded copy of the workload (independent problems => weak scaling)
-    wr = inputs.variant(w, seed_offset=1000 * rank)
-    f0, E, B, dt = inputs.make_all(wr)
+    halo_mode = args.decomp == "halo" or (args.decomp == "auto" and world > 1)
+    if halo_mode:
+        # one problem, N blocks along the periodic x axis (box and grid N times longer in x)
+        from paper_2305_01487_b200 import halo
+        wg = inputs.variant(w, name=f"{w.name}_x{world}", nx=(w.nx[0] * world, w.nx[1], w.nx[2]),
+                            xhi=(w.xlo[0] + (w.xhi[0] - w.xlo[0]) * world, w.xhi[1], w.xhi[2]))
+        dec = halo.Decomp(wg.nx, wg.bc, (world, 1, 1))
+        Eg, Bg = inputs.make_fields(wg)
+        dt = inputs.cfl_dt(wg, Eg, Bg)                       # same on every rank (global fields)
+        sl = dec.local_slices(rank)
+        E, B = (np.ascontiguousarray(a[(slice(None),) + sl]) for a in (Eg, Bg))
+        wr = inputs.variant(dec.local_workload(wg, rank), seed_offset=1000 * rank)
+        f0 = inputs.make_f0(wr)
+    else:
+        # each rank: its own seeded copy of the workload (independent problems => weak scaling)
+        wr = inputs.variant(w, seed_offset=1000 * rank)
+        f0, E, B, dt = inputs.make_all(wr)
     peaks = {}
     try:
         peaks = json.loads((ROOT / "MEASURED_PEAKS.json").read_text())
@@ -203,7 +225,13 @@ def run_mphv(args, w):
         pass
     peak_gbs, peak_src = (float(peaks["hbm_gbs"]), "measured") if "hbm_gbs" in peaks else (6650.0, "fallback")
 
-    sim = mphv.Vlasov.from_workload(wr, device=dev)
+    if halo_mode:
+        dv = halo.DistributedVlasov(wg, dec, rank, dev, force_halo=(world == 1))
+        sim = dv.sim
+        step_moments = dv.step_moments
+    else:
+        sim = mphv.Vlasov.from_workload(wr, device=dev)
+        step_moments = sim.step_moments
     sim.set_fusion(args.fusion)
     f = torch.from_numpy(f0).to(dev)
     sim.bind_f(f)
@@ -217,7 +245,7 @@ def run_mphv(args, w):
         torch.cuda.synchronize()
 
     for _ in range(max(3, args.warmup)):
-        sim.step_moments(dt, mom)
+        step_moments(dt, mom)
     barrier()
     launches0 = sim.launches
     sim.set_timing(True)
@@ -226,7 +254,7 @@ def run_mphv(args, w):
         barrier()
         e0.record()
         for _ in range(args.steps):
-            sim.step_moments(dt, mom)
+            step_moments(dt, mom)
         e1.record()
         barrier()
     ms = e0.elapsed_time(e1)
@@ -274,7 +302,10 @@ def run_mphv(args, w):
         "config": {"workload": w.name, "cells_per_gpu": w.n_cells, "bytes_per_copy_of_f": w.n_cells * 8,
                    "step": "S_x,S_y[,S_z],V_vx,V_vy,V_vz + moments n,j,P every step",
                    "l2": "inputs larger than L2 (f is %.2f GB >> 126 MB); no flush needed" % (w.n_cells * 8 / 1e9),
-                   "fusion": args.fusion, "parallelism": f"{world} independent problems" if world > 1 else "1 GPU"},
+                   "fusion": args.fusion,
+                   "parallelism": "1 GPU" if world == 1 else
+                   (f"{world} spatial blocks along periodic x, 2-layer halo exchange before S_x (NCCL send/recv), "
+                    f"{2 * sim.halo_count(0) * 8} B sent per rank per step" if halo_mode else f"{world} independent problems")},
         "clocks": clk.summary(), "gpu_launches": launches, "roofline": roofline,
     }
 
@@ -284,12 +315,22 @@ def run_mphv(args, w):
         nh = torch.empty(wr.space_shape, dtype=torch.float64).pin_memory()
         jh = torch.empty((3,) + wr.space_shape, dtype=torch.float64).pin_memory()
         Ph = torch.empty((6,) + wr.space_shape, dtype=torch.float64).pin_memory()
-        sim.run_host(fh, 1, dt, nh, jh, Ph)                     # warm-up
+        if halo_mode:
+            def run_host_step():                                # the same traffic as mphv_run_host, with the exchange
+                f.copy_(fh, non_blocking=True)
+                step_moments(dt, mom)
+                fh.copy_(f, non_blocking=True)
+                nh.copy_(mom[0], non_blocking=True); jh.copy_(mom[1], non_blocking=True); Ph.copy_(mom[2], non_blocking=True)
+                torch.cuda.synchronize()
+        else:
+            def run_host_step():
+                sim.run_host(fh, 1, dt, nh, jh, Ph)
+        run_host_step()                                         # warm-up
         barrier()
         t0 = time.perf_counter()
         e0.record()
         for _ in range(args.e2e_steps):
-            sim.run_host(fh, 1, dt, nh, jh, Ph)
+            run_host_step()
         e1.record()
         barrier()
         wall = time.perf_counter() - t0
@@ -301,7 +342,9 @@ def run_mphv(args, w):
         line["e2e"] = {"value": w.n_cells * world * args.e2e_steps / (ems * 1e-3), "unit": UNIT,
                        "h2d_bytes_per_step": w.n_cells * 8, "d2h_bytes_per_step": w.n_cells * 8 + 10 * wr.n_space * 8,
                        "ms_per_step": ems / args.e2e_steps, "steps": args.e2e_steps,
-                       "what": "mphv_run_host: pinned host f -> device, full split step, moments, f and moments -> host"}
+                       "what": ("pinned host f -> device, decomposed split step with halo exchange, moments, f and moments -> host"
+                                if halo_mode else
+                                "mphv_run_host: pinned host f -> device, full split step, moments, f and moments -> host")}
         del fh
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:

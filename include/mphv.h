@@ -109,6 +109,31 @@ int mphv_sweep_v(mphv_ctx *ctx, int dim, double dt);
  * kernel; the result is that of the unfused sequence up to fp64 rounding. */
 int mphv_step(mphv_ctx *ctx, double dt);
 
+/* The V stage of mphv_step alone: V_vx, V_vy, V_vz in that order (fused as in mphv_step), and, when
+ * n_dev is not NULL, the moments of the result (then j_dev and P_dev must be given too). With
+ * mphv_sweep_x / mphv_sweep_x_halo for the X stage this is mphv_step[_moments] taken apart, for callers
+ * that exchange boundary cells between the spatial sweeps (spatial block decomposition). */
+int mphv_stage_v(mphv_ctx *ctx, double dt, double *n_dev, double *j_dev, double *P_dev);
+
+/* ---- spatial block decomposition over several GPUs (the paper's MPI domain decomposition with
+ * boundary cells; "two boundary cells"). A context then describes ONE block; along a
+ * decomposed spatial axis its ghost cells come from the neighbouring blocks instead of the bc rule.
+ *
+ * mphv_halo_count: doubles in one halo slab of axis dim = 2 layers x (cells of the block / nx[dim]).
+ * mphv_pack_halo:  copies the two boundary layers of f at the low (side 0) or high (side 1) end of
+ *                  spatial axis dim into buf_dev (device, halo_count doubles), laid out as f with
+ *                  extent 2 along dim, layers in ascending index order. What a block packs at its
+ *                  high end is its upper neighbour's lo halo and vice versa.
+ * mphv_sweep_x_halo: S_dim(dt) as mphv_sweep_x, with the two ghost layers below the block read from
+ *                  lo_dev and the two above from hi_dev (device or peer-mapped memory, layout as
+ *                  packed). A NULL pointer marks a global OUTFLOW end (zero-gradient ghosts, R6);
+ *                  on a periodic axis both must be given (the wrap-around neighbour's layers).
+ *                  Needs max |s| < 1 (else MPHV_ERR_RANGE: whole-cell shifts would reach past the
+ *                  two boundary cells). The result on the block equals the sweep of the whole grid. */
+size_t mphv_halo_count(const mphv_ctx *ctx, int dim);
+int mphv_pack_halo(mphv_ctx *ctx, int dim, int side, double *buf_dev);
+int mphv_sweep_x_halo(mphv_ctx *ctx, int dim, double dt, const double *lo_dev, const double *hi_dev);
+
 /* Velocity moments by the midpoint rule at velocity cell centres (R9, R10):
  * n = sum f dV, j_a = sum v_a f dV, P_ab = sum v_a v_b f dV, dV = dvx dvy dvz.
  * Outputs: device, n [nz][ny][nx], j [3][...], P [6][...] (xx,xy,xz,yy,yz,zz). */

@@ -16,7 +16,7 @@ ROOT = PKG.parent
 CSRC = PKG / "csrc"
 SO = PKG / "libmphv.so"
 SOURCES = [CSRC / "mphv.cu"]
-DEPS = SOURCES + [CSRC / "mphv_kernels.cuh", ROOT / "include" / "mphv.h"]
+DEPS = SOURCES + sorted(CSRC.glob("*.cuh")) + [ROOT / "include" / "mphv.h"]
 
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-lineinfo",

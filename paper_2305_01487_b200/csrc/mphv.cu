@@ -43,11 +43,11 @@ struct mphv_ctx {
 };
 
 enum { SLOT_SX0 = 0, SLOT_SX1, SLOT_SX2, SLOT_VX, SLOT_VY, SLOT_VZ, SLOT_MOM, SLOT_VXY, SLOT_VZMOM,
-       SLOT_SHIFT, SLOT_SUM, SLOT_AMAX, SLOT_VCUBE, SLOT_VCUBE_MOM, SLOT_COUNT };
+       SLOT_SHIFT, SLOT_SUM, SLOT_AMAX, SLOT_VCUBE, SLOT_VCUBE_MOM, SLOT_PACK, SLOT_COUNT };
 static const char *const SLOT_NAMES[SLOT_COUNT] = {
     "sweep_x0", "sweep_x1", "sweep_x2", "sweep_vx", "sweep_vy", "sweep_vz", "moments",
     "fused_vx_vy", "fused_vz_moments", "shift_periodic", "sum_f", "amax_fields",
-    "fused_vx_vy_vz", "fused_vx_vy_vz_moments" };
+    "fused_vx_vy_vz", "fused_vx_vy_vz_moments", "pack_halo" };
 
 namespace {
 
@@ -604,6 +604,55 @@ int mphv_moments(mphv_ctx *c, double *n, double *j, double *P)
     if (!n || !j || !P) { set_err(c, "n_dev, j_dev or P_dev is NULL"); return MPHV_ERR_ARG; }
     if (!c->f) { set_err(c, "f not bound (mphv_bind_f)"); return MPHV_ERR_STATE; }
     return do_moments(c, n, j, P);
+}
+
+int mphv_stage_v(mphv_ctx *c, double dt, double *n, double *j, double *P)
+{
+    int st = check_common(c, dt, true);
+    if (st != MPHV_OK) return st;
+    if (n && (!j || !P)) { set_err(c, "n_dev given but j_dev or P_dev is NULL"); return MPHV_ERR_ARG; }
+    for (int d = 0; d < 3; ++d)
+        if (c->grid.nv[d] > 1 && (st = range_v(c, d, dt)) != MPHV_OK) return st;
+    return do_v_stage(c, dt, n, j, P);
+}
+
+size_t mphv_halo_count(const mphv_ctx *c, int dim)
+{
+    if (!c || dim < 0 || dim > 2 || c->grid.nx[dim] < 2) return 0;
+    return 2 * (c->nf / (size_t)c->grid.nx[dim]);
+}
+
+int mphv_pack_halo(mphv_ctx *c, int dim, int side, double *buf)
+{
+    if (!c) return MPHV_ERR_ARG;
+    if (dim < 0 || dim > 2 || c->grid.nx[dim] < 2) { set_err(c, "spatial dim %d out of range or inactive", dim); return MPHV_ERR_ARG; }
+    if (side != 0 && side != 1) { set_err(c, "side must be 0 (low end) or 1 (high end)"); return MPHV_ERR_ARG; }
+    if (!buf || ((uintptr_t)buf & 15)) { set_err(c, "buf_dev is NULL or not 16-byte aligned"); return MPHV_ERR_ARG; }
+    if (!c->f) { set_err(c, "f not bound (mphv_bind_f)"); return MPHV_ERR_STATE; }
+    const MarchArgs a = march_args_space(c, dim, 0.0);
+    const int row0 = side ? a.n - 2 : 0;
+    Timed tm(c, SLOT_PACK, 2.0 * 8.0 * (double)mphv_halo_count(c, dim));
+    if (a.inner % 2 == 0)
+        pack_halo_kernel<2><<<grid_for(a.outer * 2 * (a.inner / 2), 256), 256, 0, c->stream>>>(c->f, buf, a.outer, a.n, a.inner, row0);
+    else
+        pack_halo_kernel<1><<<grid_for(a.outer * 2 * a.inner, 256), 256, 0, c->stream>>>(c->f, buf, a.outer, a.n, a.inner, row0);
+    return after_launch(c, "pack_halo_kernel");
+}
+
+int mphv_sweep_x_halo(mphv_ctx *c, int dim, double dt, const double *lo, const double *hi)
+{
+    int st = check_common(c, dt, false);
+    if (st != MPHV_OK) return st;
+    if (dim < 0 || dim > 2 || c->grid.nx[dim] < 2) { set_err(c, "spatial dim %d out of range or inactive", dim); return MPHV_ERR_ARG; }
+    if (((uintptr_t)lo & 15) || ((uintptr_t)hi & 15)) { set_err(c, "halo buffers must be 16-byte aligned"); return MPHV_ERR_ARG; }
+    if (c->grid.bc[dim] == MPHV_BC_PERIODIC && (!lo || !hi)) {
+        set_err(c, "spatial sweep %d: a periodic axis needs both halo buffers", dim); return MPHV_ERR_ARG;
+    }
+    const double smax = max_courant_x(c, dim, dt);
+    if (!(smax < 1.0)) { set_err(c, "spatial sweep %d with halos: max |s| = %g >= 1 reaches past the two boundary cells", dim, smax); return MPHV_ERR_RANGE; }
+    MarchArgs a = march_args_space(c, dim, dt);
+    a.halo_lo = lo; a.halo_hi = hi;
+    return launch_march<KIND_SPACE, BC_HALO>(c, a);
 }
 
 int mphv_step_moments(mphv_ctx *c, double dt, double *n, double *j, double *P)

@@ -5,11 +5,9 @@
 // with oracle/ (the CPU test oracle) and includes nothing from it.
 //
 // Kernel families
-//   march_kernel     1-D PFC-3 remap along a STRIDED axis (x, y, z, vy, vz). One thread owns
-//                    VEC adjacent pencils (adjacent in the contiguous index), marches along
-//                    the axis with a register window and a U-deep register prefetch, in
-//                    place. A warp touches 32*VEC*8 contiguous bytes per march step, so
-//                    stride-N directions stay coalesced without a transpose.
+//   march2_kernel    (mphv_march.cuh) 1-D PFC-3 remap along a STRIDED axis (x, y, z, vy, vz),
+//                    in place, one thread per VEC adjacent pencils.
+//   vcube_kernel     (mphv_vcube.cuh) V_vx + V_vy [+ V_vz + moments] per velocity plane stream.
 //   vx_kernel        remap along the CONTIGUOUS axis vx: one thread owns CH consecutive cells
 //                    of a row, reads its 2+2 halo through L1, all loads -> barrier -> stores.
 //   moments_kernel   one CTA per spatial cell: separable accumulation along vz, then
@@ -22,7 +20,7 @@
 
 namespace mphv {
 
-enum { BC_PER = 0, BC_OUT = 1, BC_WALL = 2 };
+enum { BC_PER = 0, BC_OUT = 1, BC_WALL = 2, BC_HALO = 3 };
 enum { KIND_SPACE = 0, KIND_VEL = 1 };
 
 struct GridDev {
@@ -45,6 +43,10 @@ struct MarchArgs {
     double *mom;            // fused moments: per-CTA partials [ns*tiles][10] (vz sweep only) or null
     int tiles, per_tile;    // CTA tiling of the fused-moments variant
     double dV;
+    // BC_HALO (spatial block decomposition): the two ghost layers below / above the block,
+    // each [outer][2][inner] (layers in ascending index order). NULL = that end is a global outflow
+    // end (zero-gradient ghosts, R6).
+    const double *halo_lo, *halo_hi;
     GridDev g;
 };
 
@@ -170,148 +172,7 @@ __device__ __forceinline__ void block_reduce_sum(double (&val)[NV], double *smem
     }
 }
 
-// ---------------------------------------------------------------- march kernel
-// In-place remap with |s| < 1 (k = 0). Window (g_{i-1}, g_i, g_{i+1}, g_{i+2}) in registers;
-// buf/nxt hold the next 2U loads so that U independent loads per thread are always in flight.
-template <int VEC, int U, int KIND, int BC, bool MOM>
-__global__ void __launch_bounds__(256)
-march_kernel(const MarchArgs p)
-{
-    typedef V<VEC> T;
-    __shared__ double red[MOM ? 10 * 32 : 1];
-    const long long innerV = p.inner / VEC;
-    long long o, ev;
-    bool active;
-    if (MOM) {
-        // CTA-tiled: blockIdx.x = o * tiles + tile, a CTA never straddles spatial cells
-        o = blockIdx.x / p.tiles;
-        const int tile = blockIdx.x - (int)o * p.tiles;
-        const int lt = threadIdx.x;
-        ev = (long long)tile * p.per_tile + lt;
-        active = lt < p.per_tile && ev < innerV;
-    } else {
-        const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-        active = t < p.outer * innerV;
-        o = t / innerV;
-        ev = t - o * innerV;
-        if (!active) return;
-    }
-    double mom[10];
-    if (MOM) {
-#pragma unroll
-        for (int k = 0; k < 10; ++k) mom[k] = 0.0;
-    }
-    if (active) {
-    const long long e0 = ev * VEC;
-    const int n = p.n;
-    const long long stride = p.inner;
-    double *base = p.f + (o * n) * stride + e0;
-
-    Courant cn[VEC];
-#pragma unroll
-    for (int l = 0; l < VEC; ++l) cn[l] = make_courant(pencil_courant<KIND>(p, o, e0 + l));
-
-    T f0s, f1s;                                  // originals of cells 0, 1 (periodic wrap)
-    T gm2, gm1, c0, c1v;
-    c0 = ldv<VEC>(base);
-    c1v = ldv<VEC>(base + stride);
-    f0s = c0; f1s = c1v;
-    if (BC == BC_PER) {
-        gm2 = ldv<VEC>(base + (long long)(n - 2) * stride);
-        gm1 = ldv<VEC>(base + (long long)(n - 1) * stride);
-    } else if (BC == BC_OUT) {
-        gm2 = c0; gm1 = c0;
-    } else {
-#pragma unroll
-        for (int l = 0; l < VEC; ++l) { gm2.v[l] = 0.0; gm1.v[l] = 0.0; }
-    }
-
-    auto fetch = [&](int i) -> T {
-        if (i < n) return ldv<VEC>(base + (long long)i * stride);
-        if (BC == BC_PER) return (i == n) ? f0s : f1s;
-        if (BC == BC_OUT) return ldv<VEC>(base + (long long)(n - 1) * stride);
-        T z;
-#pragma unroll
-        for (int l = 0; l < VEC; ++l) z.v[l] = 0.0;
-        return z;
-    };
-
-    T buf[U], nxt[U];
-#pragma unroll
-    for (int u = 0; u < U; ++u) buf[u] = fetch(2 + u);
-
-    // flux through the low face -1/2 (zero for the closed velocity box, R7)
-    T phiprev;
-#pragma unroll
-    for (int l = 0; l < VEC; ++l) {
-        if (BC == BC_WALL) phiprev.v[l] = 0.0;
-        else {
-            const bool ps = cn[l].pos;
-            phiprev.v[l] = face_flux(ps ? gm2.v[l] : c1v.v[l], ps ? gm1.v[l] : c0.v[l],
-                                     ps ? c0.v[l] : gm1.v[l], cn[l].sf, cn[l].c1, cn[l].c2);
-        }
-    }
-    T a1 = gm1;                                  // g_{i-1}
-    double s0[VEC], s1[VEC], s2[VEC];            // sum f, sum vz f, sum vz^2 f along the march (MOM)
-#pragma unroll
-    for (int l = 0; l < VEC; ++l) { s0[l] = 0.0; s1[l] = 0.0; s2[l] = 0.0; }
-
-    for (int i0 = 0; i0 < n; i0 += U) {
-#pragma unroll
-        for (int u = 0; u < U; ++u) nxt[u] = fetch(i0 + 2 + U + u);
-#pragma unroll
-        for (int u = 0; u < U; ++u) {
-            const int i = i0 + u;
-            if (i < n) {
-                const T c2v = buf[u];            // g_{i+2}
-                T out;
-#pragma unroll
-                for (int l = 0; l < VEC; ++l) {
-                    const bool ps = cn[l].pos;
-                    double phi = face_flux(ps ? a1.v[l] : c2v.v[l], ps ? c0.v[l] : c1v.v[l],
-                                           ps ? c1v.v[l] : c0.v[l], cn[l].sf, cn[l].c1, cn[l].c2);
-                    if (BC == BC_WALL && i == n - 1) phi = 0.0;
-                    out.v[l] = c0.v[l] + (phiprev.v[l] - phi);
-                    phiprev.v[l] = phi;
-                }
-                stv<VEC>(base + (long long)i * stride, out);
-                if (MOM) {
-                    const double vz = vcentre(p.g, 2, i);
-#pragma unroll
-                    for (int l = 0; l < VEC; ++l) {
-                        const double tz = vz * out.v[l];
-                        s0[l] += out.v[l]; s1[l] += tz; s2[l] = fma(vz, tz, s2[l]);
-                    }
-                }
-                a1 = c0; c0 = c1v; c1v = c2v;
-            }
-        }
-#pragma unroll
-        for (int u = 0; u < U; ++u) buf[u] = nxt[u];
-    }
-    if (MOM) {
-        // thread's pencils sit at (jy, jx) = divmod(e0 + l, nvx): combine with vx, vy
-#pragma unroll
-        for (int l = 0; l < VEC; ++l) {
-            const long long e = e0 + l;
-            const int jy = (int)(e / p.g.nv[0]), jx = (int)(e - (long long)jy * p.g.nv[0]);
-            const double vx = vcentre(p.g, 0, jx), vy = vcentre(p.g, 1, jy);
-            const double x0 = vx * s0[l], y0 = vy * s0[l];
-            mom[0] += s0[l];
-            mom[1] += x0; mom[2] += y0; mom[3] += s1[l];
-            mom[4] = fma(vx, x0, mom[4]); mom[5] = fma(vx, y0, mom[5]); mom[6] = fma(vx, s1[l], mom[6]);
-            mom[7] = fma(vy, y0, mom[7]); mom[8] = fma(vy, s1[l], mom[8]); mom[9] += s2[l];
-        }
-    }
-    }   // active
-    if (MOM) {
-        block_reduce_sum<10>(mom, red);
-        if (threadIdx.x == 0) {
-#pragma unroll
-            for (int k = 0; k < 10; ++k) p.mom[(long long)blockIdx.x * 10 + k] = mom[k];
-        }
-    }
-}
+// ---------------------------------------------------------------- march kernel: mphv_march.cuh
 
 // Sums the per-CTA partial moments of the fused V_vz kernel in fixed order and scales by dV.
 __global__ void __launch_bounds__(256)

@@ -86,6 +86,17 @@ march2_kernel(const MarchArgs p)
             gm2 = ldv<VEC>(base + (long long)(n - 2) * stride);
             gm1 = ldv<VEC>(base + (long long)(n - 1) * stride);
         }
+        T hn0, hn1;                                  // BC_HALO: ghost layers above the block
+        if (BC == BC_HALO) {
+            if (p.halo_lo) {
+                const double *h = p.halo_lo + (o * 2) * stride + e0;
+                gm2 = ldv<VEC>(h); gm1 = ldv<VEC>(h + stride);
+            }
+            if (p.halo_hi) {
+                const double *h = p.halo_hi + (o * 2) * stride + e0;
+                hn0 = ldv<VEC>(h); hn1 = ldv<VEC>(h + stride);
+            }
+        }
         T pre[2 * U - 1];
 #pragma unroll
         for (int u = 0; u < 2 * U - 1; ++u)
@@ -97,7 +108,7 @@ march2_kernel(const MarchArgs p)
             for (int u = 0; u < U; ++u) bufA[u] = ldv<VEC>(nextp + (long long)u * stride);
         }
         const T F0 = G0, F1 = G1;                    // originals of cells 0, 1 (periodic wrap)
-        if (BC == BC_OUT) { gm2 = G0; gm1 = G0; }
+        if (BC == BC_OUT || (BC == BC_HALO && !p.halo_lo)) { gm2 = G0; gm1 = G0; }
         if (BC == BC_WALL) {
 #pragma unroll
             for (int l = 0; l < VEC; ++l) { gm2.v[l] = 0.0; gm1.v[l] = 0.0; }
@@ -182,7 +193,9 @@ march2_kernel(const MarchArgs p)
         T gn0, gn1;                                  // g_n, g_{n+1}
         if (BC == BC_PER) { gn0 = F0; gn1 = F1; }
         else if (BC == BC_OUT) { gn0 = G1; gn1 = G1; }                  // G1 = g_{n-1} here
-        else {
+        else if (BC == BC_HALO) {
+            if (p.halo_hi) { gn0 = hn0; gn1 = hn1; } else { gn0 = G1; gn1 = G1; }
+        } else {
 #pragma unroll
             for (int l = 0; l < VEC; ++l) { gn0.v[l] = 0.0; gn1.v[l] = 0.0; }
         }
@@ -213,6 +226,25 @@ march2_kernel(const MarchArgs p)
             for (int k = 0; k < 10; ++k) p.mom[(long long)blockIdx.x * 10 + k] = mom[k];
         }
     }
+}
+
+// ---------------------------------------------------------------- halo pack
+// Copies the two boundary layers of f at one end of a spatial axis (f viewed as [outer][n][inner])
+// into buf [outer][2][inner], layers in ascending index order: row0 = 0 (low end) or n-2 (high end).
+// 16-byte vector copies when inner is even.
+template <int VEC>
+__global__ void __launch_bounds__(256)
+pack_halo_kernel(const double *__restrict__ f, double *__restrict__ buf, long long outer, int n,
+                 long long inner, int row0)
+{
+    const long long innerV = inner / VEC;
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= outer * 2 * innerV) return;
+    const long long ol = t / innerV;                 // (o, layer)
+    const long long ev = t - ol * innerV;
+    const long long o = ol >> 1;
+    const int layer = (int)(ol & 1);
+    stv<VEC>(buf + ol * inner + ev * VEC, ldv<VEC>(f + (o * n + row0 + layer) * inner + ev * VEC));
 }
 
 }  // namespace mphv

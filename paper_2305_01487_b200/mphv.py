@@ -27,6 +27,7 @@ SYMBOLS = (
     "mphv_moments", "mphv_step_moments", "mphv_run_host", "mphv_sum_f", "mphv_launch_count",
     "mphv_set_fusion", "mphv_strerror", "mphv_last_error",
     "mphv_set_timing", "mphv_timing_slots", "mphv_get_timing",
+    "mphv_stage_v", "mphv_halo_count", "mphv_pack_halo", "mphv_sweep_x_halo",
 )
 
 
@@ -78,6 +79,10 @@ def lib() -> C.CDLL:
         "mphv_timing_slots": (i32, []),
         "mphv_get_timing": (i32, [vp, i32, C.c_char_p, C.c_size_t, C.POINTER(dbl),
                                   C.POINTER(C.c_uint64), C.POINTER(dbl)]),
+        "mphv_stage_v": (i32, [vp, dbl, vp, vp, vp]),
+        "mphv_halo_count": (C.c_size_t, [vp, i32]),
+        "mphv_pack_halo": (i32, [vp, i32, i32, vp]),
+        "mphv_sweep_x_halo": (i32, [vp, i32, dbl, vp, vp]),
         "mphv_strerror": (C.c_char_p, [i32]),
         "mphv_last_error": (C.c_char_p, [vp]),
     }
@@ -161,6 +166,22 @@ def mphv_moments(ctx, n_dev: int, j_dev: int, P_dev: int):
 
 def mphv_step_moments(ctx, dt: float, n_dev: int, j_dev: int, P_dev: int):
     _check(ctx, lib().mphv_step_moments(ctx, float(dt), n_dev, j_dev, P_dev))
+
+
+def mphv_stage_v(ctx, dt: float, n_dev=None, j_dev=None, P_dev=None):
+    _check(ctx, lib().mphv_stage_v(ctx, float(dt), n_dev, j_dev, P_dev))
+
+
+def mphv_halo_count(ctx, dim: int) -> int:
+    return int(lib().mphv_halo_count(ctx, int(dim)))
+
+
+def mphv_pack_halo(ctx, dim: int, side: int, buf_dev: int):
+    _check(ctx, lib().mphv_pack_halo(ctx, int(dim), int(side), buf_dev))
+
+
+def mphv_sweep_x_halo(ctx, dim: int, dt: float, lo_dev=None, hi_dev=None):
+    _check(ctx, lib().mphv_sweep_x_halo(ctx, int(dim), float(dt), lo_dev, hi_dev))
 
 
 def mphv_run_host(ctx, f_host: int, nsteps: int, dt: float, n_host=None, j_host=None, P_host=None):
@@ -273,6 +294,26 @@ class Vlasov:
         n, j, P = out if out is not None else self.alloc_moments()
         mphv_step_moments(self.ctx, dt, n.data_ptr(), j.data_ptr(), P.data_ptr())
         return n, j, P
+
+    def stage_v(self, dt, out=None):
+        """The V stage alone; with out = (n, j, P) tensors the moments of the result are written too."""
+        if out is None:
+            mphv_stage_v(self.ctx, dt)
+            return None
+        n, j, P = out
+        mphv_stage_v(self.ctx, dt, n.data_ptr(), j.data_ptr(), P.data_ptr())
+        return out
+
+    def halo_count(self, dim) -> int:
+        return mphv_halo_count(self.ctx, dim)
+
+    def pack_halo(self, dim, side, buf):
+        mphv_pack_halo(self.ctx, dim, side, self._dev(buf, self.halo_count(dim)))
+
+    def sweep_x_halo(self, dim, dt, lo=None, hi=None):
+        cnt = self.halo_count(dim)
+        mphv_sweep_x_halo(self.ctx, dim, dt, None if lo is None else self._dev(lo, cnt),
+                          None if hi is None else self._dev(hi, cnt))
 
     def sum_f(self) -> float:
         torch = self.torch

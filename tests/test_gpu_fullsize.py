@@ -1,0 +1,95 @@
+"""GPU parity at BASELINE.json's full sizes (configs 2, 3, 4), in the launch configuration
+bench.py times (mphv_step_moments, default fusion level), on SAMPLED outputs the oracle computes
+one by one.
+
+One full split step at spatial cell c reads f only inside the box c +- 2 cells per spatial axis
+(S_x, S_y, S_z reach two cells each at |s| < 1; the V stage and the moments are
+local to the spatial cell). So for each sampled cell the oracle advances the 5 x 5 (x 5) spatial
+block around it -- indices wrapped on periodic axes, clamped on outflow axes, which is exactly
+the boundary rule R6 -- and its centre cell is the full-grid result, whatever boundary rule the
+small block itself uses. Samples include the domain corners and edges, the sheet centre and
+seeded random cells. Properties that hold at any size (f >= 0, finite moments, total mass against
+the density moment) are checked on the whole array."""
+import itertools
+
+import numpy as np
+import pytest
+
+from parity_util import TOL_SWEEP, local_scale
+
+pytestmark = pytest.mark.gpu
+
+
+def block_indices(w, cell):
+    """Per spatial axis d: the five indices cell[d]-2 .. cell[d]+2 under the axis' boundary rule."""
+    out = []
+    for d in range(3):
+        n = w.nx[d]
+        if n == 1:
+            out.append(np.array([0]))
+            continue
+        idx = np.arange(cell[d] - 2, cell[d] + 3)
+        out.append(idx % n if w.bc[d] == 0 else np.clip(idx, 0, n - 1))
+    return out
+
+
+def sample_cells(w, rng, n_random=6):
+    """Domain corners and edge cells (first, second, last index per active axis in 2-D; corners in
+    3-D), the centre, and seeded random cells."""
+    three_d = sum(1 for n in w.nx if n > 1) == 3
+    axes = [[0] if n == 1 else ([0, n - 1] if three_d else [0, 1, n // 2, n - 1]) for n in w.nx]
+    cells = set(itertools.product(*axes))
+    cells.add(tuple(n // 2 for n in w.nx))
+    want = len(cells) + n_random
+    while len(cells) < want:
+        cells.add(tuple(int(rng.integers(0, n)) for n in w.nx))
+    return sorted(cells)
+
+
+@pytest.mark.parametrize("index", [2, 3, 4])
+def test_full_size_step_moments_on_sampled_cells(orc, index):
+    import torch
+    from paper_2305_01487_b200 import inputs, mphv
+    w = inputs.config(index)
+    f0, E, B, dt = inputs.make_all(w)
+    sim = mphv.Vlasov.from_workload(w)
+    f = torch.from_numpy(f0).cuda()
+    sim.bind_f(f)
+    sim.set_fields(torch.from_numpy(E).cuda(), torch.from_numpy(B).cuda())
+    n_g, j_g, P_g = sim.step_moments(dt)
+    torch.cuda.synchronize()
+
+    # whole-array properties
+    assert float(f.min()) >= 0.0, "positivity"
+    assert bool(torch.isfinite(f).all())
+    dV = w.dv(0) * w.dv(1) * w.dv(2)
+    mass_f = sim.sum_f() * dV
+    mass_n = float(n_g.sum(dtype=torch.float64))
+    assert abs(mass_f - mass_n) <= 1e-12 * abs(mass_f), "sum of the density moment = dV * sum of f"
+
+    rng = np.random.default_rng(w.seed + 31)
+    sub_nx = tuple(5 if w.nx[d] > 1 else 1 for d in range(3))
+    grid = orc.Grid(sub_nx, w.nv, (1, 1, 1))
+    xlo = tuple(0.0 for _ in range(3))
+    xhi = tuple(w.dx(d) * sub_nx[d] if w.nx[d] > 1 else 1.0 for d in range(3))
+    box = orc.Box(xlo, xhi, w.vlo, w.vhi)
+    n_g, j_g, P_g = n_g.cpu().numpy(), j_g.cpu().numpy(), P_g.cpu().numpy()
+    worst = 0.0
+    for cell in sample_cells(w, rng):
+        ix, iy, iz = block_indices(w, cell)
+        blk = np.ascontiguousarray(f0[np.ix_(iz, iy, ix)])
+        Eb = np.ascontiguousarray(E[np.ix_([0, 1, 2], iz, iy, ix)])
+        Bb = np.ascontiguousarray(B[np.ix_([0, 1, 2], iz, iy, ix)])
+        orc.step(blk, grid, box, w.q_over_m, Eb, Bb, dt)
+        n_r, j_r, P_r = orc.moments(blk, grid, box)
+        c = tuple(2 if w.nx[d] > 1 else 0 for d in range(3))
+        ref = blk[c[2], c[1], c[0]]
+        got = f[cell[2], cell[1], cell[0]].cpu().numpy()
+        scale = np.maximum(local_scale(ref, 0), 1e-300)            # last-swept axis of the cube: vz
+        err = float(np.max(np.abs(got - ref) / scale))
+        worst = max(worst, err)
+        assert err <= TOL_SWEEP, f"{w.name} cell {cell}: step err {err:.3e}"
+        sc = abs(P_r[0][c[2], c[1], c[0]]) + abs(P_r[3][c[2], c[1], c[0]]) + abs(P_r[5][c[2], c[1], c[0]]) + abs(n_r[c[2], c[1], c[0]])
+        for a_g, a_r in [(n_g[None], n_r[None]), (j_g, j_r), (P_g, P_r)]:
+            d = np.abs(a_g[:, cell[2], cell[1], cell[0]] - a_r[:, c[2], c[1], c[0]])
+            assert np.max(d) <= 1e-12 * sc, f"{w.name} cell {cell}: moments"
