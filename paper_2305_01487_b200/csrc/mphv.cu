@@ -5,6 +5,7 @@
 #include "mphv_kernels.cuh"
 #include "mphv_vcube.cuh"
 #include "mphv_march.cuh"
+#include "mphv_vstage.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -30,6 +31,7 @@ struct mphv_ctx {
     int mom_tiles, mom_per_tile, mom_block;   // CTA tiling of the fused V_vz + moments kernel
     int sm_count;
     int vxy_T, vxy_grid; size_t vxy_smem;     // fused V_vx + V_vy plane kernel launch shape (0 = unsupported)
+    int vs_T, vs_grid, vs_variant; size_t vs_smem;   // second-generation whole-V-stage kernel (T = 0: unsupported)
     int cube_T, cube_grid, cube_variant, plane_grid; size_t cube_smem, plane_smem;  // whole-V-stage cube kernel launch shape (T = 0: unsupported)
     uint64_t launches;
     int fusion;
@@ -221,6 +223,23 @@ void *plane_fn(int variant)
     }
 }
 
+// second-generation whole-V-stage kernel (mphv_vstage.cuh): same shape specialisations
+template <bool MOM> void *vstage_fn(int variant)
+{
+    switch (variant) {
+    case CUBE_40: return (void *)vstage_kernel<3, MOM, 40, 40, 416, 1>;
+    case CUBE_32: return (void *)vstage_kernel<2, MOM, 32, 32, 256, 2>;
+    default:      return (void *)vstage_kernel<3, MOM, 0, 0, 512, 1>;
+    }
+}
+int vstage_ns(int variant) { return variant == CUBE_32 ? 2 : 3; }
+
+size_t vstage_smem_bytes(int nvx, int nvy, int nvz, int ns)
+{
+    const size_t cells = (size_t)nvx * nvy, xcells = (size_t)nvx * (nvy + 4);
+    return (ns * 2 * cells + VS_NXB * 2 * xcells + nvz + 320) * sizeof(double) + (ns + 2) * sizeof(uint64_t);
+}
+
 size_t cube_smem_bytes(int nvx, int nvy, int nvz, int ns, bool reduce)
 {
     const size_t cells = (size_t)nvx * nvy, xcells = (size_t)nvx * (nvy + 4);
@@ -248,6 +267,27 @@ int launch_vcube(mphv_ctx *c, double dt, bool with_vz, double *n, double *j, dou
                                      with_vz ? c->cube_smem : c->plane_smem, c->stream);
     if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(c, e, "vcube_kernel launch"); }
     return after_launch(c, "vcube_kernel");
+}
+
+// V_vx, V_vy, V_vz (+ moments if n != NULL) in one pass over f, two planes per pipeline iteration
+int launch_vstage(mphv_ctx *c, double dt, double *n, double *j, double *P)
+{
+    CubeArgs a;
+    std::memset(&a, 0, sizeof a);
+    a.f = c->f;
+    a.ns = (long long)c->ns;
+    a.nvx = c->grid.nv[0]; a.nvy = c->grid.nv[1]; a.nvz = c->grid.nv[2];
+    a.dt = dt;
+    a.E = c->E; a.B = c->B;
+    a.n = n; a.j = j; a.P = P;
+    a.dV = c->dv[0] * c->dv[1] * c->dv[2];
+    a.g = c->gd;
+    Timed tm(c, n ? SLOT_VCUBE_MOM : SLOT_VCUBE, (n ? 56.0 : 48.0) * (double)c->nf);
+    void *fn = n ? vstage_fn<true>(c->vs_variant) : vstage_fn<false>(c->vs_variant);
+    void *args[] = { &a };
+    cudaError_t e = cudaLaunchKernel(fn, dim3((unsigned)c->vs_grid), dim3((unsigned)c->vs_T), args, c->vs_smem, c->stream);
+    if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(c, e, "vstage_kernel launch"); }
+    return after_launch(c, "vstage_kernel");
 }
 
 MarchArgs march_args_space(const mphv_ctx *c, int d, double dt)
@@ -336,6 +376,7 @@ int do_v_stage(mphv_ctx *c, double dt, double *n, double *j, double *P)
 {
     int st;
     const bool ax = c->grid.nv[0] > 1, ay = c->grid.nv[1] > 1, az = c->grid.nv[2] > 1;
+    if (c->fusion >= 2 && c->vs_T > 0) return launch_vstage(c, dt, n, j, P);
     if (c->fusion >= 2 && c->cube_T > 0) return launch_vcube(c, dt, true, n, j, P);
     if (c->fusion && c->cube_T > 0 && c->plane_grid > 0) {
         if ((st = launch_vcube(c, dt, false, nullptr, nullptr, nullptr)) != MPHV_OK) return st;
@@ -499,6 +540,24 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
                     c->plane_grid = (int)pg; c->plane_smem = psmem;
                 }
             }
+        }
+        cudaGetLastError();
+    }
+    c->vs_T = 0;
+    if (grid->nv[0] % 4 == 0 && grid->nv[1] % 4 == 0 && grid->nv[2] >= 4 && grid->nv[2] % 2 == 0) {
+        const int nvx = grid->nv[0], nvy = grid->nv[1], nvz = grid->nv[2];
+        const int T = (nvy * (nvx / 4) + 31) / 32 * 32;
+        const int variant = (nvx == 40 && nvy == 40) ? CUBE_40 : (nvx == 32 && nvy == 32) ? CUBE_32 : CUBE_GEN;
+        const size_t smem = vstage_smem_bytes(nvx, nvy, nvz, vstage_ns(variant));
+        int max_optin = 0, per_sm = 0;
+        cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+        if (T <= 512 && smem <= (size_t)max_optin &&
+            cudaFuncSetAttribute(vstage_fn<true>(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess &&
+            cudaFuncSetAttribute(vstage_fn<false>(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess &&
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, vstage_fn<true>(variant), T, smem) == cudaSuccess && per_sm > 0) {
+            long long g = (long long)per_sm * c->sm_count;
+            if (g > (long long)c->ns) g = (long long)c->ns;
+            c->vs_T = T; c->vs_smem = smem; c->vs_grid = (int)g; c->vs_variant = variant;
         }
         cudaGetLastError();
     }
