@@ -43,8 +43,8 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs index (default 3, headline)")
     ap.add_argument("--impl", default="mphv", choices=["mphv", "reference"])
-    ap.add_argument("--fusion", type=int, default=1, choices=[0, 1, 2],
-                    help="mphv_set_fusion level: 0 one kernel per sweep, 1 pairwise fused, 2 whole V stage in one kernel; default 1")
+    ap.add_argument("--fusion", type=int, default=1, choices=[0, 1, 2, 3],
+                    help="mphv_set_fusion level: 0 one kernel per sweep, 1 pairwise fused, 2 whole V stage in one kernel, 3 also S_x+S_y in one kernel; default 1")
     ap.add_argument("--decomp", default="auto", choices=["auto", "halo", "none"],
                     help="'halo' = one spatially decomposed problem with neighbour exchange (the default for N > 1; "
                          "at N = 1 the block is its own periodic neighbour), 'none' = N independent problems "

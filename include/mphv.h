@@ -109,6 +109,11 @@ int mphv_sweep_v(mphv_ctx *ctx, int dim, double dt);
  * kernel; the result is that of the unfused sequence up to fp64 rounding. */
 int mphv_step(mphv_ctx *ctx, double dt);
 
+/* The X stage of mphv_step alone: S_x, S_y, S_z in that order (fused as in mphv_step), inactive
+ * dimensions skipped; range checks as mphv_sweep_x, all before the first sweep is enqueued. With
+ * mphv_stage_v this gives callers true Strang splitting, X(dt/2) V(dt) X(dt/2). */
+int mphv_stage_x(mphv_ctx *ctx, double dt);
+
 /* The V stage of mphv_step alone: V_vx, V_vy, V_vz in that order (fused as in mphv_step), and, when
  * n_dev is not NULL, the moments of the result (then j_dev and P_dev must be given too). With
  * mphv_sweep_x / mphv_sweep_x_halo for the X stage this is mphv_step[_moments] taken apart, for callers
@@ -173,9 +178,11 @@ int mphv_get_timing(mphv_ctx *ctx, int slot, char *name, size_t name_cap, double
 
 /* Tuning knob for experiments and tests. level 0 = one kernel per sweep; 1 = pairwise fused
  * kernels (V_vx+V_vy per velocity plane, V_vz+moments; the default, fastest measured on B200);
- * 2 = the whole V stage (three sweeps and the moments) in one pass over f. Levels 1 and 2 fall
- * back to lower-level kernels for grids their kernels do not cover (nvx, nvy not multiples of 4
- * resp. 2, fewer than 3 velocity dimensions). Results agree up to fp64 rounding at every level. */
+ * 2 = the whole V stage (three sweeps and the moments) in one pass over f; 3 = level 2 plus the
+ * spatial sweeps S_x and S_y in one pass over f. Levels 1..3 fall back to lower-level kernels for
+ * grids their kernels do not cover (nvx, nvy not multiples of 4 resp. 2, fewer than 3 velocity
+ * dimensions; nx not a multiple of 4, nvel not a multiple of 8, |s| >= 1 on a periodic axis).
+ * Results agree up to fp64 rounding at every level. */
 int mphv_set_fusion(mphv_ctx *ctx, int level);
 
 const char *mphv_strerror(int code);

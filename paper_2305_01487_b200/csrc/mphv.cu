@@ -6,6 +6,7 @@
 #include "mphv_vcube.cuh"
 #include "mphv_march.cuh"
 #include "mphv_vstage.cuh"
+#include "mphv_sxy.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -32,24 +33,25 @@ struct mphv_ctx {
     int sm_count;
     int vxy_T, vxy_grid; size_t vxy_smem;     // fused V_vx + V_vy plane kernel launch shape (0 = unsupported)
     int vs_T, vs_grid, vs_variant; size_t vs_smem;   // second-generation whole-V-stage kernel (T = 0: unsupported)
+    int sxy_T, sxy_C; size_t sxy_smem;               // fused S_x + S_y kernel (T = 0: unsupported)
     int cube_T, cube_grid, cube_variant, plane_grid; size_t cube_smem, plane_smem;  // whole-V-stage cube kernel launch shape (T = 0: unsupported)
     uint64_t launches;
     int fusion;
     int timing;
     struct Pending { int slot; cudaEvent_t e0, e1; };
     std::vector<Pending> *pending;
-    double slot_ms[16];
-    uint64_t slot_launches[16];
-    double slot_bytes[16];
+    double slot_ms[24];
+    uint64_t slot_launches[24];
+    double slot_bytes[24];
     char err[512];
 };
 
 enum { SLOT_SX0 = 0, SLOT_SX1, SLOT_SX2, SLOT_VX, SLOT_VY, SLOT_VZ, SLOT_MOM, SLOT_VXY, SLOT_VZMOM,
-       SLOT_SHIFT, SLOT_SUM, SLOT_AMAX, SLOT_VCUBE, SLOT_VCUBE_MOM, SLOT_PACK, SLOT_COUNT };
+       SLOT_SHIFT, SLOT_SUM, SLOT_AMAX, SLOT_VCUBE, SLOT_VCUBE_MOM, SLOT_PACK, SLOT_SXY, SLOT_COUNT };
 static const char *const SLOT_NAMES[SLOT_COUNT] = {
     "sweep_x0", "sweep_x1", "sweep_x2", "sweep_vx", "sweep_vy", "sweep_vz", "moments",
     "fused_vx_vy", "fused_vz_moments", "shift_periodic", "sum_f", "amax_fields",
-    "fused_vx_vy_vz", "fused_vx_vy_vz_moments", "pack_halo" };
+    "fused_vx_vy_vz", "fused_vx_vy_vz_moments", "pack_halo", "fused_sx_sy" };
 
 namespace {
 
@@ -288,6 +290,45 @@ int launch_vstage(mphv_ctx *c, double dt, double *n, double *j, double *P)
     cudaError_t e = cudaLaunchKernel(fn, dim3((unsigned)c->vs_grid), dim3((unsigned)c->vs_T), args, c->vs_smem, c->stream);
     if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(c, e, "vstage_kernel launch"); }
     return after_launch(c, "vstage_kernel");
+}
+
+// S_x then S_y in one pass over f (mphv_sxy.cuh)
+const int SXY_NR = 6;                   // ring depth: SXY_NR - 1 rows in flight per CTA
+
+void *sxy_fn(int C, int bcx, int bcy)
+{
+#define SXY_PICK(CC, TM, MB) \
+    (bcx == MPHV_BC_PERIODIC ? (bcy == MPHV_BC_PERIODIC ? (void *)sxy_kernel<CC, SXY_NR, BC_PER, BC_PER, TM, MB> \
+                                                         : (void *)sxy_kernel<CC, SXY_NR, BC_PER, BC_OUT, TM, MB>) \
+                             : (bcy == MPHV_BC_PERIODIC ? (void *)sxy_kernel<CC, SXY_NR, BC_OUT, BC_PER, TM, MB> \
+                                                         : (void *)sxy_kernel<CC, SXY_NR, BC_OUT, BC_OUT, TM, MB>))
+    return C == 16 ? SXY_PICK(16, 512, 1) : SXY_PICK(8, 256, 2);
+#undef SXY_PICK
+}
+
+size_t sxy_smem_bytes(int C, int nx, int T, bool per_y)
+{
+    const size_t rowd = C == 16 ? sxy_row_doubles<16>(nx) : sxy_row_doubles<8>(nx);
+    return (SXY_NR * rowd + (per_y ? 8 * (size_t)T : 0)) * sizeof(double);
+}
+
+int launch_sxy(mphv_ctx *c, double dt)
+{
+    SxyArgs a;
+    std::memset(&a, 0, sizeof a);
+    a.f = c->f;
+    a.nx = c->grid.nx[0]; a.ny = c->grid.nx[1];
+    a.nvel = (long long)c->nvel;
+    a.chunks = (int)(c->nvel / (size_t)c->sxy_C);
+    a.dt = dt; a.dx = c->dx[0]; a.dy = c->dx[1];
+    a.g = c->gd;
+    Timed tm(c, SLOT_SXY, 32.0 * (double)c->nf);
+    void *fn = sxy_fn(c->sxy_C, c->grid.bc[0], c->grid.bc[1]);
+    void *args[] = { &a };
+    const unsigned grid = (unsigned)((long long)c->grid.nx[2] * a.chunks);
+    cudaError_t e = cudaLaunchKernel(fn, dim3(grid), dim3((unsigned)c->sxy_T), args, c->sxy_smem, c->stream);
+    if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(c, e, "sxy_kernel launch"); }
+    return after_launch(c, "sxy_kernel");
 }
 
 MarchArgs march_args_space(const mphv_ctx *c, int d, double dt)
@@ -561,6 +602,32 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
         }
         cudaGetLastError();
     }
+    c->sxy_T = 0;
+    if (grid->nx[0] >= 8 && grid->nx[0] % 4 == 0 && grid->nx[1] >= 4) {
+        const int nx = grid->nx[0];
+        int C = 0;
+#ifndef MPHV_SXY_PREFER_C8
+        if (c->nvel % 16 == 0 && (nx / 4) * 16 <= 512) C = 16;
+        else
+#endif
+        if (c->nvel % 8 == 0 && (nx / 4) * 8 <= 256) C = 8;
+        if (C) {
+            const int T = (nx / 4) * C;
+            size_t smem = 0;
+            int max_optin = 0;
+            cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+            bool ok = true;
+            for (int by = 0; by < 2 && ok; ++by) {
+                const size_t sm = sxy_smem_bytes(C, nx, T, by == MPHV_BC_PERIODIC);
+                if (by == grid->bc[1]) smem = sm;
+                for (int bx = 0; bx < 2 && ok; ++bx)
+                    ok = sm <= (size_t)max_optin &&
+                         cudaFuncSetAttribute(sxy_fn(C, bx, by), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) == cudaSuccess;
+            }
+            if (ok) { c->sxy_T = T; c->sxy_C = C; c->sxy_smem = smem; }
+        }
+        cudaGetLastError();
+    }
     e = cudaMalloc(&c->ws, (10 * c->ns * (1 + (size_t)c->mom_tiles) + SUM_BLOCKS + 8) * sizeof(double));
     if (e != cudaSuccess) { set_err(nullptr, "cudaMalloc workspace: %s", cudaGetErrorString(e)); cudaGetLastError(); delete c->pending; delete c; return nullptr; }
     return c;
@@ -646,12 +713,24 @@ static int step_checks(mphv_ctx *c, double dt)
     return MPHV_OK;
 }
 
+static int x_stage(mphv_ctx *c, double dt)
+{
+    int st;
+    int d0 = 0;
+    if (c->fusion >= 3 && c->sxy_T > 0 && max_courant_x(c, 0, dt) < 1.0 && max_courant_x(c, 1, dt) < 1.0) {
+        if ((st = launch_sxy(c, dt)) != MPHV_OK) return st;        // S_x, S_y in one pass
+        d0 = 2;
+    }
+    for (int d = d0; d < 3; ++d)
+        if (c->grid.nx[d] > 1 && (st = do_sweep_x(c, d, dt)) != MPHV_OK) return st;
+    return MPHV_OK;
+}
+
 static int step_impl(mphv_ctx *c, double dt, double *n, double *j, double *P)
 {
     int st = step_checks(c, dt);
     if (st != MPHV_OK) return st;
-    for (int d = 0; d < 3; ++d)
-        if (c->grid.nx[d] > 1 && (st = do_sweep_x(c, d, dt)) != MPHV_OK) return st;
+    if ((st = x_stage(c, dt)) != MPHV_OK) return st;
     return do_v_stage(c, dt, n, j, P);
 }
 
@@ -663,6 +742,15 @@ int mphv_moments(mphv_ctx *c, double *n, double *j, double *P)
     if (!n || !j || !P) { set_err(c, "n_dev, j_dev or P_dev is NULL"); return MPHV_ERR_ARG; }
     if (!c->f) { set_err(c, "f not bound (mphv_bind_f)"); return MPHV_ERR_STATE; }
     return do_moments(c, n, j, P);
+}
+
+int mphv_stage_x(mphv_ctx *c, double dt)
+{
+    int st = check_common(c, dt, false);
+    if (st != MPHV_OK) return st;
+    for (int d = 0; d < 3; ++d)
+        if (c->grid.nx[d] > 1 && (st = range_x(c, d, dt)) != MPHV_OK) return st;
+    return x_stage(c, dt);
 }
 
 int mphv_stage_v(mphv_ctx *c, double dt, double *n, double *j, double *P)
@@ -760,7 +848,7 @@ int mphv_set_timing(mphv_ctx *c, int enabled)
     if (!c) return MPHV_ERR_ARG;
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     drain_timing(c, false);
-    for (int i = 0; i < 16; ++i) { c->slot_ms[i] = 0.0; c->slot_launches[i] = 0; c->slot_bytes[i] = 0.0; }
+    for (int i = 0; i < 24; ++i) { c->slot_ms[i] = 0.0; c->slot_launches[i] = 0; c->slot_bytes[i] = 0.0; }
     c->timing = enabled ? 1 : 0;
     return MPHV_OK;
 }
@@ -786,7 +874,7 @@ uint64_t mphv_launch_count(const mphv_ctx *c) { return c ? c->launches : 0; }
 int mphv_set_fusion(mphv_ctx *c, int enabled)
 {
     if (!c) return MPHV_ERR_ARG;
-    c->fusion = enabled < 0 ? 0 : (enabled > 2 ? 2 : enabled);
+    c->fusion = enabled < 0 ? 0 : (enabled > 3 ? 3 : enabled);
     return MPHV_OK;
 }
 

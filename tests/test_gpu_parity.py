@@ -97,7 +97,7 @@ def test_each_sweep_matches_oracle(torch_cuda, mphv, orc, nx, nv, bc, sign):
 
 @pytest.mark.parametrize("nx,nv,bc", SHAPES + [((4, 4, 1), (40, 40, 8), (0, 1, 0)), ((4, 4, 1), (20, 36, 4), (0, 0, 0)),
                                             ((4, 4, 1), (4, 4, 4), (0, 1, 0)), ((4, 4, 1), (64, 8, 1), (0, 1, 0))])
-@pytest.mark.parametrize("fusion", [0, 1, 2])
+@pytest.mark.parametrize("fusion", [0, 1, 2, 3])
 def test_full_step_and_moments_fused_and_unfused(torch_cuda, mphv, orc, nx, nv, bc, fusion):
     """mphv_step_moments (fused plane kernel vx+vy, fused vz+moments when fusion is on) against
     oracle step + oracle moments, ragged and odd shapes included (odd extents fall back to the
@@ -153,7 +153,7 @@ def test_limiter_active_data_matches_oracle(torch_cuda, mphv, orc):
     assert rel_err(g, p.f_ref, AX_V[2]) <= TOL_SWEEP
 
 
-@pytest.mark.parametrize("fusion", [0, 1, 2])
+@pytest.mark.parametrize("fusion", [0, 1, 2, 3])
 def test_config0_landau_20_steps_and_moments(torch_cuda, mphv, orc, fusion):
     from paper_2305_01487_b200 import inputs
     w = inputs.config(0)
@@ -187,7 +187,7 @@ def check_moments(p, orc, g):
             k += 1
 
 
-@pytest.mark.parametrize("fusion", [0, 1, 2])
+@pytest.mark.parametrize("fusion", [0, 1, 2, 3])
 def test_config1_harris_steps_and_moments(torch_cuda, mphv, orc, fusion):
     from paper_2305_01487_b200 import inputs
     w = inputs.config(1)
@@ -205,6 +205,59 @@ def test_config1_harris_steps_and_moments(torch_cuda, mphv, orc, fusion):
     assert abs(m_gpu - m_ref) <= TOL_MASS * abs(m_ref)
     assert abs(p.sim.sum_f() - m_ref) <= TOL_MASS * abs(m_ref), "device-side sum"
     check_moments(p, orc, g)
+
+
+SXY_SHAPES = [
+    # nx, nv, bc : nvel % 16 == 0 (128-byte chunks) and nvel % 16 == 8 (64-byte chunks), every
+    # combination of periodic / outflow on x and y, ragged thread counts, 3-D (S_z stays a march)
+    ((12, 10, 1), (12, 10, 8), (0, 1, 0)),
+    ((12, 10, 1), (12, 10, 8), (1, 0, 0)),
+    ((16, 9, 1), (6, 4, 1), (0, 0, 0)),
+    ((16, 9, 1), (6, 4, 1), (1, 1, 0)),
+    ((8, 4, 1), (4, 4, 4), (0, 1, 0)),
+    ((36, 8, 1), (40, 12, 6), (0, 1, 0)),
+    ((8, 6, 4), (8, 6, 4), (0, 1, 0)),
+    ((64, 7, 1), (8, 4, 4), (0, 1, 0)),
+    ((128, 6, 1), (4, 4, 1), (0, 0, 0)),
+]
+
+
+@pytest.mark.parametrize("nx,nv,bc", SXY_SHAPES)
+@pytest.mark.parametrize("sign", [1.0, -1.0])
+def test_stage_x_fused_matches_oracle_sweeps(torch_cuda, mphv, orc, nx, nv, bc, sign):
+    """mphv_stage_x at fusion level 3 (S_x and S_y in one pass, sxy_kernel) against the oracle's
+    S_x, S_y, S_z in order (R5), both signs of dt, CFL 0.85."""
+    w = small_workload(nx, nv, bc)
+    p = Pair(torch_cuda, mphv, orc, w, fusion=3)
+    dt = sign * 1.7 * p.dt
+    for rep in range(2):
+        last = 0
+        for d in range(3):
+            if w.nx[d] > 1:
+                orc.sweep_x(p.f_ref, p.grid, p.box, d, dt)
+                last = d
+        n0 = p.sim.launches
+        p.sim.stage_x(dt)
+        assert p.sim.launches - n0 == (2 if w.nx[2] > 1 else 1), "the fused kernel must be the one that ran"
+        g = p.gpu()
+        assert rel_err(g, p.f_ref, AX_X[last]) <= 2 * TOL_SWEEP, f"rep {rep}"
+        assert rel_err(g, p.f_ref, AX_X[0]) <= 2 * TOL_SWEEP
+        p.set_f(p.f_ref)
+
+
+def test_stage_x_then_stage_v_is_step(torch_cuda, mphv, orc):
+    """Strang pieces: stage_x(dt/2), stage_v(dt), stage_x(dt/2) against the oracle's sweeps."""
+    w = small_workload((12, 8, 1), (8, 8, 8))
+    for fusion in (0, 3):
+        p = Pair(torch_cuda, mphv, orc, w, fusion=fusion)
+        for d in (0, 1):
+            orc.sweep_x(p.f_ref, p.grid, p.box, d, 0.5 * p.dt)
+        for d in range(3):
+            orc.sweep_v(p.f_ref, p.grid, p.box, w.q_over_m, p.E, p.B, d, p.dt)
+        for d in (0, 1):
+            orc.sweep_x(p.f_ref, p.grid, p.box, d, 0.5 * p.dt)
+        p.sim.stage_x(0.5 * p.dt); p.sim.stage_v(p.dt); p.sim.stage_x(0.5 * p.dt)
+        assert rel_err(p.gpu(), p.f_ref, AX_X[1]) <= 3 * TOL_SWEEP
 
 
 def test_step_moments_equals_step_then_moments(torch_cuda, mphv, orc):
