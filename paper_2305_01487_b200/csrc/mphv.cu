@@ -236,10 +236,10 @@ template <bool MOM> void *vstage_fn(int variant)
 }
 int vstage_ns(int variant) { return variant == CUBE_32 ? 2 : 3; }
 
-size_t vstage_smem_bytes(int nvx, int nvy, int nvz, int ns)
+size_t vstage_smem_bytes(int nvx, int nvy, int nvz, int ns, int T)
 {
     const size_t cells = (size_t)nvx * nvy, xcells = (size_t)nvx * (nvy + 4);
-    return (ns * 2 * cells + VS_NXB * 2 * xcells + nvz + 320) * sizeof(double) + (ns + 2) * sizeof(uint64_t);
+    return (ns * 2 * cells + VS_NXB * 2 * xcells + nvz + 320 + 8 * (size_t)T) * sizeof(double) + (ns + 2) * sizeof(uint64_t);
 }
 
 size_t cube_smem_bytes(int nvx, int nvy, int nvz, int ns, bool reduce)
@@ -589,7 +589,7 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
         const int nvx = grid->nv[0], nvy = grid->nv[1], nvz = grid->nv[2];
         const int T = (nvy * (nvx / 4) + 31) / 32 * 32;
         const int variant = (nvx == 40 && nvy == 40) ? CUBE_40 : (nvx == 32 && nvy == 32) ? CUBE_32 : CUBE_GEN;
-        const size_t smem = vstage_smem_bytes(nvx, nvy, nvz, vstage_ns(variant));
+        const size_t smem = vstage_smem_bytes(nvx, nvy, nvz, vstage_ns(variant), T);
         int max_optin = 0, per_sm = 0;
         cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
         if (T <= 512 && smem <= (size_t)max_optin &&

@@ -166,7 +166,8 @@ sxy_kernel(const SxyArgs p)
         }
         dst += row_stride;
     };
-    for (; k < K; ++k) {
+#pragma unroll 3
+    for (; k < K; ++k) {                             // unrolled by the period of the (G0, G1, nw) rotation
         double nw[4];
         produce(k, nw);
         ystep(nw);

@@ -45,7 +45,8 @@ vstage_kernel(const CubeArgs p)
     double *xb = ring + (size_t)NS * 2 * cells;                         // [VS_NXB][2][nvy + 4][nvx]
     double *vzt = xb + (size_t)VS_NXB * 2 * xcells;                     // [nvz] vz centres
     double *red = vzt + nvz;                                            // [10][32]
-    uint64_t *bars = reinterpret_cast<uint64_t *>(red + 320);           // [NS] TMA full, [2] xbar
+    double2 *zc = reinterpret_cast<double2 *>(red + 320);               // [4][T] V_vz slope coefficients of the thread's pencils
+    uint64_t *bars = reinterpret_cast<uint64_t *>(zc + 4 * (size_t)blockDim.x);   // [NS] TMA full, [2] xbar
 
     const long long c_begin = (p.ns * (long long)blockIdx.x) / gridDim.x;
     const long long c_end = (p.ns * ((long long)blockIdx.x + 1)) / gridDim.x;
@@ -89,11 +90,12 @@ vstage_kernel(const CubeArgs p)
     // per-cube linear forms of the Courant numbers: s = a + vz b
     double ax = 0.0, bx = 0.0, ay = 0.0, by = 0.0;
     // V_vz march state of this thread's 4 pencils (rows r0..r0+3 of column jx)
-    double zs[4], zx[4], zy[4];                      // s, coefficient of lim(g_{j+1}-g_j), of lim(g_{j-1}-g_j)
+    double zs[4];                                    // s; the coefficients of lim(g_{j+1}-g_j), lim(g_{j-1}-g_j) live in zc
+    double2 *const zcp = zc + tid;                   // (shared memory, written and read by this thread only)
     double G0[4], G1[4], Q[4], E[4];                 // g_i, g_{i+1}, Q_i, E_i = Q_{i-1} - Q_i
     double P0 = 0.0, Q1 = 0.0, Q2 = 0.0, Z1 = 0.0, Z2 = 0.0, ZQ = 0.0;   // moment sums (see header)
 #pragma unroll
-    for (int m = 0; m < 4; ++m) { zs[m] = zx[m] = zy[m] = 0.0; G0[m] = G1[m] = Q[m] = E[m] = 0.0; }
+    for (int m = 0; m < 4; ++m) { zs[m] = 0.0; G0[m] = G1[m] = Q[m] = E[m] = 0.0; }
 
     // One march step for the 4 pencils: nw = g_{i+2} arrives, Q_{i+1} is formed, cell i is finished
     // and stored to plane i (po). MODE 0: interior; 1: i = nvz-2 (Q_{i+1} sits in front of the high
@@ -104,7 +106,8 @@ vstage_kernel(const CubeArgs p)
 #pragma unroll
         for (int m = 0; m < 4; ++m) {
             const bool pos = __double2hiint(zs[m]) >= 0;
-            double qn = march_q(G0[m], G1[m], nw[m], zx[m], zy[m]);
+            const double2 zxy = zcp[m * blockDim.x];
+            double qn = march_q(G0[m], G1[m], nw[m], zxy.x, zxy.y);
             if (MODE == 1 && pos) qn = 0.0;
             if (MODE == 2 && !pos) qn = 0.0;
             const double en = Q[m] - qn;
@@ -193,8 +196,7 @@ vstage_kernel(const CubeArgs p)
                 courant_poly(s, c1, nc2);
                 const bool pos = __double2hiint(s) >= 0;
                 zs[m] = s;
-                zx[m] = pos ? c1 : nc2;
-                zy[m] = pos ? nc2 : c1;
+                zcp[m * blockDim.x] = pos ? make_double2(c1, nc2) : make_double2(nc2, c1);
             }
             P0 = Q1 = Q2 = Z1 = Z2 = ZQ = 0.0;
         }
@@ -202,15 +204,24 @@ vstage_kernel(const CubeArgs p)
             const double *xsrc = xb + (size_t)(ib % VS_NXB) * 2 * xcells + xr_off;
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
-                const double *xi = xsrc + h * xcells;
-                double w[8];
-#pragma unroll
-                for (int r = 0; r < 8; ++r) w[r] = xi[r * nvx];
                 const int jz = 2 * jB + h;
                 const double s = fma(vzt[jz], by, ay);
                 double c1, nc2, nw[4];
                 courant_poly(s, c1, nc2);
-                remap4(w, s, c1, nc2, ylo_wall, yhi_wall, nw);
+                // the 7-row window starts one row later for s < 0: lanes of either sign run the same code
+                const bool pos = __double2hiint(s) >= 0;
+                const double *xi = xsrc + h * xcells;
+                const double *xw = pos ? xi : xi + nvx;
+                const double ccx = pos ? c1 : nc2, ccy = pos ? nc2 : c1;
+                double w[7], q[5];
+#pragma unroll
+                for (int r = 0; r < 7; ++r) w[r] = xw[r * nvx];
+#pragma unroll
+                for (int r = 0; r < 5; ++r) q[r] = march_q(w[r], w[r + 1], w[r + 2], ccx, ccy);
+                if (ylo_wall) q[0] = 0.0;            // closed box (R7): the wall faces carry no flux
+                if (yhi_wall) q[4] = 0.0;
+#pragma unroll
+                for (int r = 0; r < 4; ++r) nw[r] = fma(s, q[r] - q[r + 1], xi[(r + 2) * nvx]);
                 if (jB == 0) {
                     if (h == 0) {
 #pragma unroll
@@ -220,7 +231,8 @@ vstage_kernel(const CubeArgs p)
                         for (int m = 0; m < 4; ++m) {                    // g_1: Q_0, E_0 (face -1/2 carries no flux)
                             const bool pos = __double2hiint(zs[m]) >= 0;
                             G1[m] = nw[m];
-                            double q0 = march_q(0.0, G0[m], G1[m], zx[m], zy[m]);
+                            const double2 zxy = zcp[m * blockDim.x];
+                            double q0 = march_q(0.0, G0[m], G1[m], zxy.x, zxy.y);
                             if (!pos) q0 = 0.0;
                             Q[m] = q0; E[m] = -q0;
                         }
