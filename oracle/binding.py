@@ -101,6 +101,17 @@ def lib() -> C.CDLL:
         L.orc_sum.restype = C.c_double
         L.orc_f_count.argtypes = [C.POINTER(_CGrid)]
         L.orc_f_count.restype = C.c_size_t
+        d3, d9 = C.c_double * 3, C.c_double * 9
+        L.orc_boris_map.argtypes = [C.c_double, d3, d3, C.c_double, d9, d3]
+        L.orc_boris_map.restype = None
+        L.orc_backsub_foot.argtypes = [d9, d3, C.c_int, d3]
+        L.orc_backsub_foot.restype = C.c_double
+        L.orc_sweep_pencil_faces.argtypes = [dp, dp, C.c_int, dp]
+        L.orc_sweep_pencil_faces.restype = C.c_int
+        L.orc_sweep_v_backsub.argtypes = L.orc_sweep_v.argtypes
+        L.orc_sweep_v_backsub.restype = C.c_int
+        L.orc_step_backsub.argtypes = L.orc_step.argtypes
+        L.orc_step_backsub.restype = C.c_int
         L.orc_num_threads.argtypes = []
         L.orc_num_threads.restype = C.c_int
         _lib = L
@@ -159,6 +170,56 @@ def step(f: np.ndarray, grid: Grid, box: Box, q_over_m: float, E: np.ndarray, B:
     st = lib().orc_step(_p(f), C.byref(g), C.byref(b), float(q_over_m), _p(E), _p(B), float(dt), C.byref(net))
     if st != OK:
         raise ValueError(f"orc_step status {st}")
+    return net.value
+
+
+def boris_map(q_over_m: float, E, B, dt: float):
+    """Boris map of one spatial cell, v_new = R v_old + c: returns (R 3x3, c 3)."""
+    d3, d9 = C.c_double * 3, C.c_double * 9
+    R, c = d9(), d3()
+    lib().orc_boris_map(float(q_over_m), d3(*map(float, E)), d3(*map(float, B)), float(dt), R, c)
+    return np.array(R[:]).reshape(3, 3), np.array(c[:])
+
+
+def backsub_foot(R, c, dim: int, v) -> float:
+    """Foot coordinate of backsubstituted sweep `dim` at the point v (see mphv_oracle.c)."""
+    d3, d9 = C.c_double * 3, C.c_double * 9
+    Rf = [float(x) for x in np.asarray(R).reshape(9)]
+    return float(lib().orc_backsub_foot(d9(*Rf), d3(*map(float, c)), int(dim), d3(*map(float, v))))
+
+
+def sweep_pencil_faces(pencil, s_face):
+    """Closed-box 1-D PFC-3 remap with one Courant number per face (n + 1 of them)."""
+    a = np.ascontiguousarray(pencil, dtype=np.float64)
+    sf = np.ascontiguousarray(s_face, dtype=np.float64)
+    assert sf.size == a.size + 1
+    out = np.empty_like(a)
+    st = lib().orc_sweep_pencil_faces(_p(a), _p(out), a.size, _p(sf))
+    if st != OK:
+        raise ValueError(f"orc_sweep_pencil_faces status {st}")
+    return out
+
+
+def sweep_v_backsub(f: np.ndarray, grid: Grid, box: Box, q_over_m: float, E: np.ndarray, B: np.ndarray,
+                    dim: int, dt: float) -> None:
+    _check_f(f, grid)
+    assert E.size == 3 * grid.n_space and B.size == 3 * grid.n_space
+    g, b = grid.c(), box.c()
+    st = lib().orc_sweep_v_backsub(_p(f), C.byref(g), C.byref(b), float(q_over_m), _p(E), _p(B), dim, float(dt))
+    if st != OK:
+        raise ValueError(f"orc_sweep_v_backsub status {st}")
+
+
+def step_backsub(f: np.ndarray, grid: Grid, box: Box, q_over_m: float, E: np.ndarray, B: np.ndarray,
+                 dt: float) -> float:
+    """One full split step with the backsubstituted V stage, in place; returns the net spatial outflow."""
+    _check_f(f, grid)
+    assert E.size == 3 * grid.n_space and B.size == 3 * grid.n_space
+    net = C.c_double(0.0)
+    g, b = grid.c(), box.c()
+    st = lib().orc_step_backsub(_p(f), C.byref(g), C.byref(b), float(q_over_m), _p(E), _p(B), float(dt), C.byref(net))
+    if st != OK:
+        raise ValueError(f"orc_step_backsub status {st}")
     return net.value
 
 

@@ -25,7 +25,9 @@
  * Pins (tests/test_oracle_pins.py, all -m "not gpu"): integer-Courant exact
  * translation, exact-rational remap brute force, quadratic exactness, mass
  * conservation, positivity, mirror symmetry, free streaming, gyration closure,
- * uniform-E shift, Maxwellian and hand-summed moments.
+ * uniform-E shift, Maxwellian and hand-summed moments; for the backsubstituted V
+ * stage (R15): exact-rational composition of the three foot maps, reduction to the
+ * plain sweeps at B = 0, gyration closure at large angle, conservation, positivity.
  * PARITY UNPINNED against the authors' own implementation: PAPER.md prints no
  * value of their scheme's output anywhere.
  *
@@ -374,6 +376,225 @@ int orc_moments(const double *f, const orc_grid *g, const orc_box *b,
         for (int a = 0; a < 3; ++a) j_out[(size_t)a * ns + c] = (double)(m1[a] * dV);
         for (int a = 0; a < 6; ++a) P_out[(size_t)a * ns + c] = (double)(m2[a] * dV);
     }
+    return ORC_OK;
+}
+
+/* ==========================================================================
+ * Backsubstitution velocity update.
+ * P:L137 (sec. 4.1): "The velocity space splitting is realized via
+ * backsubstitution [27]"; "For the Lagrangian treatment, we developed the
+ * backsubstitution method [27]". PAPER.md prints no formula; the statement below
+ * is the reading R15 of DESIGN.md, derived from what the method has to achieve:
+ * three 1-D shifts along vx, vy, vz whose COMPOSITION is the exact characteristic
+ * foot of the velocity-space part of eq. (1) over dt with frozen fields, instead
+ * of the three plain shifts a_d dt, which commit an O((q/m)|B| dt) splitting error.
+ *
+ * Characteristic map. The velocity part of eq. (1) is dv/dt = (q/m)(E + v x B).
+ * Over one step it is integrated by the Boris rotation (half kick, rotation
+ * about B by the angle theta with tan(theta/2) = |t|, half kick), an affine map
+ *     v_new = R v_old + c,   h = (q/m) dt / 2,  t = h B,  s = 2 t / (1 + |t|^2),
+ *     v- = v_old + h E;  v' = v- + v- x t;  v+ = v- + v' x s;  v_new = v+ + h E,
+ * so R = I + S + S T with (T u) = u x t, (S u) = u x s, and c = (I + R) h E.
+ * R is a proper rotation (the Cayley form of the rotation about B).
+ *
+ * Backsubstitution. Let V = (X, Y, Z) be the foot of v = (vx, vy, vz): v = R V + c.
+ * The three sweeps  f1(vx,Y,Z) = f0(X,Y,Z),  f2(vx,vy,Z) = f1(vx,Y,Z),
+ * f3(vx,vy,vz) = f2(vx,vy,Z)  compose to f3(v) = f0(V) if every sweep knows its foot
+ * coordinate as a function of the coordinates of the array it WRITES:
+ *   sweep 1 (vx):  X = (vx - c_x - R_xy Y - R_xz Z) / R_xx        (row x of v = R V + c)
+ *   sweep 2 (vy):  Y = (vy - c_y - R_yx (vx - c_x - R_xz Z)/R_xx - R_yz Z) / (R_yy - R_yx R_xy / R_xx)
+ *                                                                 (row y, X substituted back)
+ *   sweep 3 (vz):  Z = R_xz (vx - c_x) + R_yz (vy - c_y) + R_zz (vz - c_z)   (row z of V = R^T (v - c))
+ * ("backsubstitution": the already-final coordinates are substituted back into the rows of the map).
+ * Each is a 1-D remap along its own axis whose displacement is an affine function of the
+ * position ALONG the pencil. In flux form (PFC, the same limiter and polynomial as c-4/c-5)
+ * the face at coordinate xi is displaced to its foot: the flux through it is the integral of
+ * the reconstruction over [foot(xi), xi], i.e. the c-5 flux with the face's own Courant number
+ *     s_face = (xi - foot(xi)) / dv_d,   |s_face| < 1 required,
+ * and the two wall faces carry no flux (R7). The three 1-D maps have Jacobians
+ * 1/R_xx, 1/(R_yy - R_yx R_xy/R_xx), R_zz whose product is 1 (R_zz is the cofactor
+ * R_xx R_yy - R_xy R_yx of a rotation), so the conservative composition transports f as the
+ * advective one does.
+ * ========================================================================== */
+
+/* Boris map of one spatial cell: v_new = R v_old + c. R row-major [9]. */
+void orc_boris_map(double q_over_m, const double E[3], const double B[3], double dt,
+                   double R[9], double c[3])
+{
+    const double h = q_over_m * dt / 2.0;
+    const double t[3] = { h * B[0], h * B[1], h * B[2] };
+    const double t2 = t[0] * t[0] + t[1] * t[1] + t[2] * t[2];
+    const double s[3] = { 2.0 * t[0] / (1.0 + t2), 2.0 * t[1] / (1.0 + t2), 2.0 * t[2] / (1.0 + t2) };
+    /* (T u)_x = u_y t_z - u_z t_y, ... : matrices of u -> u x t and u -> u x s */
+    const double T[9] = { 0.0, t[2], -t[1],  -t[2], 0.0, t[0],  t[1], -t[0], 0.0 };
+    const double S[9] = { 0.0, s[2], -s[1],  -s[2], 0.0, s[0],  s[1], -s[0], 0.0 };
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) {
+            double st = 0.0;
+            for (int k = 0; k < 3; ++k) st += S[3 * i + k] * T[3 * k + j];
+            R[3 * i + j] = (i == j ? 1.0 : 0.0) + S[3 * i + j] + st;
+        }
+    const double hE[3] = { h * E[0], h * E[1], h * E[2] };
+    for (int i = 0; i < 3; ++i)
+        c[i] = hE[i] + (R[3 * i] * hE[0] + R[3 * i + 1] * hE[1] + R[3 * i + 2] * hE[2]);
+}
+
+/* Foot coordinate of sweep `dim` at the point v (v[dim] = position along the pencil, the other
+ * two entries = coordinates of the array the sweep writes, see the table above). */
+double orc_backsub_foot(const double R[9], const double c[3], int dim, const double v[3])
+{
+    if (dim == 0)
+        return (v[0] - c[0] - R[1] * v[1] - R[2] * v[2]) / R[0];
+    if (dim == 1) {
+        const double D = R[4] - R[3] * R[1] / R[0];
+        return (v[1] - c[1] - R[3] * (v[0] - c[0] - R[2] * v[2]) / R[0] - R[5] * v[2]) / D;
+    }
+    return R[2] * (v[0] - c[0]) + R[5] * (v[1] - c[1]) + R[8] * (v[2] - c[2]);
+}
+
+/* 1-D PFC-3 remap with one Courant number per face: s_face[i + 1] belongs to face i+1/2,
+ * i = -1 .. n-1; closed box (empty ghosts, the two wall faces carry no flux). c-4, c-5 with
+ * alpha (beta) = |s_face|; |s_face| < 1 on the interior faces. in, out must not alias. */
+int orc_sweep_pencil_faces(const double *in, double *out, int n, const double *s_face)
+{
+    if (!in || !out || !s_face || n < 1) return ORC_ERR_ARG;
+    for (int i = 0; i + 1 < n; ++i)
+        if (!(fabs(s_face[i + 1]) < 1.0)) return ORC_ERR_RANGE;
+    double *phi = (double *)malloc((size_t)(n + 1) * sizeof(double));
+    if (!phi) return ORC_ERR_ARG;
+#define G(i) fetch(in, n, (i), ORC_BC_WALL)
+    for (long i = -1; i < n; ++i) {
+        const double s = s_face[i + 1];
+        double ph;
+        if (s >= 0.0) {
+            const double frac = s;
+            const double c1 = ((1.0 - frac) * (2.0 - frac)) / 6.0;
+            const double c2 = ((1.0 - frac) * (1.0 + frac)) / 6.0;
+            double Lp = slope_plus(G(i), G(i + 1));
+            double Lm = slope_minus(G(i - 1), G(i));
+            ph = frac * ((G(i) + c1 * Lp) + c2 * Lm);
+        } else {
+            const double frac = -s;
+            const double c1 = ((1.0 - frac) * (2.0 - frac)) / 6.0;
+            const double c2 = ((1.0 - frac) * (1.0 + frac)) / 6.0;
+            double Lm = slope_minus(G(i), G(i + 1));
+            double Lp = slope_plus(G(i + 1), G(i + 2));
+            ph = -frac * ((G(i + 1) - c1 * Lm) - c2 * Lp);
+        }
+        phi[i + 1] = ph;
+    }
+    phi[0] = 0.0; phi[n] = 0.0;                       /* closed velocity box (R7) */
+    for (long i = 0; i < n; ++i) out[i] = in[i] + (phi[i] - phi[i + 1]);
+#undef G
+    free(phi);
+    return ORC_OK;
+}
+
+/* Courant numbers of the n+1 faces of the pencil of sweep `dim` through (v[da], v[db]) */
+static void backsub_faces(const orc_grid *g, const orc_box *b, const double R[9], const double c[3],
+                          int dim, double v[3], double *s_face)
+{
+    const int n = g->nv[dim];
+    const double dv = v_width(g, b, dim);
+    for (int i = -1; i < n; ++i) {
+        const double xi = b->vlo[dim] + ((double)(i + 1)) * dv;      /* face i+1/2 */
+        v[dim] = xi;
+        s_face[i + 1] = (xi - orc_backsub_foot(R, c, dim, v)) / dv;
+    }
+}
+
+/*
+ * Backsubstituted velocity sweep along dim (0: vx, 1: vy, 2: vz) of the velocity step dt.
+ * The three sweeps must be applied in the order vx, vy, vz (the table above). Needs all three
+ * velocity dimensions active.
+ */
+int orc_sweep_v_backsub(double *f, const orc_grid *g, const orc_box *b, double q_over_m,
+                        const double *E, const double *B, int dim, double dt)
+{
+    if (!f || !E || !B || !grid_ok(g, b) || dim < 0 || dim > 2) return ORC_ERR_ARG;
+    if (g->nv[0] < 2 || g->nv[1] < 2 || g->nv[2] < 2) return ORC_ERR_ARG;
+    if (!(dt == dt) || isinf(dt)) return ORC_ERR_ARG;
+    const int n = g->nv[dim];
+    const size_t ns = n_space(g), nvel = n_vel(g);
+    size_t vstride[3] = { 1, (size_t)g->nv[0], (size_t)g->nv[0] * g->nv[1] };
+    const size_t stride = vstride[dim];
+    const int da = (dim + 1) % 3, db = (dim + 2) % 3;
+
+    /* range check first: a failed call leaves f untouched */
+    {
+        double *sf = (double *)malloc((size_t)(n + 1) * sizeof(double));
+        if (!sf) return ORC_ERR_ARG;
+        for (size_t cc = 0; cc < ns; ++cc) {
+            double Ec[3] = { E[cc], E[ns + cc], E[2 * ns + cc] };
+            double Bc[3] = { B[cc], B[ns + cc], B[2 * ns + cc] };
+            double R[9], c[3];
+            orc_boris_map(q_over_m, Ec, Bc, dt, R, c);
+            for (int ja = 0; ja < g->nv[da]; ++ja)
+                for (int jb = 0; jb < g->nv[db]; ++jb) {
+                    double v[3];
+                    v[da] = v_centre(g, b, da, ja); v[db] = v_centre(g, b, db, jb);
+                    backsub_faces(g, b, R, c, dim, v, sf);
+                    for (int i = 0; i + 1 < n; ++i)
+                        if (!(fabs(sf[i + 1]) < 1.0)) { free(sf); return ORC_ERR_RANGE; }
+                }
+        }
+        free(sf);
+    }
+
+    int status = ORC_OK;
+#pragma omp parallel
+    {
+        double *pin = (double *)malloc((size_t)n * sizeof(double));
+        double *pout = (double *)malloc((size_t)n * sizeof(double));
+        double *sf = (double *)malloc((size_t)(n + 1) * sizeof(double));
+#pragma omp for schedule(static)
+        for (long long cc = 0; cc < (long long)ns; ++cc) {
+            size_t cell = (size_t)cc;
+            double Ec[3] = { E[cell], E[ns + cell], E[2 * ns + cell] };
+            double Bc[3] = { B[cell], B[ns + cell], B[2 * ns + cell] };
+            double R[9], c[3];
+            orc_boris_map(q_over_m, Ec, Bc, dt, R, c);
+            double *cube = f + cell * nvel;
+            for (int ja = 0; ja < g->nv[da]; ++ja)
+                for (int jb = 0; jb < g->nv[db]; ++jb) {
+                    double v[3];
+                    v[da] = v_centre(g, b, da, ja); v[db] = v_centre(g, b, db, jb);
+                    backsub_faces(g, b, R, c, dim, v, sf);
+                    size_t base = (size_t)ja * vstride[da] + (size_t)jb * vstride[db];
+                    for (int i = 0; i < n; ++i) pin[i] = cube[base + (size_t)i * stride];
+                    int st = orc_sweep_pencil_faces(pin, pout, n, sf);
+                    if (st != ORC_OK) {
+#pragma omp critical
+                        status = st;
+                        continue;
+                    }
+                    for (int i = 0; i < n; ++i) cube[base + (size_t)i * stride] = pout[i];
+                }
+        }
+        free(pin); free(pout); free(sf);
+    }
+    return status;
+}
+
+/* Full split step with the backsubstituted V stage: S_x, S_y, S_z (c-7), then the three
+ * backsubstituted sweeps vx, vy, vz of the same dt. */
+int orc_step_backsub(double *f, const orc_grid *g, const orc_box *b, double q_over_m,
+                     const double *E, const double *B, double dt, double *net_out)
+{
+    if (!grid_ok(g, b)) return ORC_ERR_ARG;
+    double net = 0.0;
+    for (int d = 0; d < 3; ++d)
+        if (g->nx[d] > 1) {
+            double part = 0.0;
+            int st = orc_sweep_x(f, g, b, d, dt, &part);
+            if (st != ORC_OK) return st;
+            net += part;
+        }
+    for (int d = 0; d < 3; ++d) {
+        int st = orc_sweep_v_backsub(f, g, b, q_over_m, E, B, d, dt);
+        if (st != ORC_OK) return st;
+    }
+    if (net_out) *net_out = net;
     return ORC_OK;
 }
 
