@@ -198,12 +198,16 @@ def _quarter_turn_error(orc, n, N, backsub):
 
 
 def test_b5_quarter_gyration_has_no_splitting_error(orc):
-    # the face displacement is |v| theta / dv < 1: N >= 6 / dv * pi/2
-    e32 = _quarter_turn_error(orc, 32, 64, True)
-    e64 = _quarter_turn_error(orc, 64, 128, True)
-    plain64 = _quarter_turn_error(orc, 64, 128, False)
-    assert e64 < 0.25 * e32 and e64 < 2e-2, (e32, e64)             # interpolation error only, converging
-    assert plain64 > 3 * e64, (plain64, e64)                       # the plain sweeps keep an O(b) error
+    # the face displacement is |v| theta / dv < 1: N >= (6 / dv) pi/2 = 25 (n = 32), 50 (n = 64)
+    e32 = _quarter_turn_error(orc, 32, 28, True)
+    e64 = _quarter_turn_error(orc, 64, 56, True)
+    e64_half_angle = _quarter_turn_error(orc, 64, 112, True)
+    plain64 = _quarter_turn_error(orc, 64, 56, False)
+    plain64_half_angle = _quarter_turn_error(orc, 64, 112, False)
+    assert e64 < e32 / 5 and e64 < 6e-3, (e32, e64)                # interpolation error only: ~third order in dv
+    assert abs(e64_half_angle - e64) < 0.2 * e64                   # ... and independent of the angle per step
+    assert plain64 > 3 * e64, (plain64, e64)                       # the plain sweeps add an O(b) splitting error
+    assert plain64_half_angle < 0.65 * plain64                     # ... which falls with the angle per step
 
 
 def test_b6_conservation_and_positivity_general_fields(orc):
