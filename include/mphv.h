@@ -176,6 +176,21 @@ int mphv_timing_slots(void);
 int mphv_get_timing(mphv_ctx *ctx, int slot, char *name, size_t name_cap, double *total_ms,
                     uint64_t *launches, double *alg_bytes_per_launch);
 
+/* Mode of the V stage. MPHV_V_PLAIN (default; BASELINE.json north_star): three plain 1-D sweeps with
+ * the Courant numbers a_d dt / dv_d, a = (q/m)(E + v x B) at the cell centres. MPHV_V_BACKSUB: "The
+ * velocity space splitting is realized via backsubstitution" (sec. 4.1; reading R15 of
+ * DESIGN.md): the three sweeps vx, vy, vz displace every cell FACE to the foot coordinate of the Boris
+ * map of the cell (half kick, rotation about B, half kick over dt), each sweep knowing the coordinates
+ * the later sweeps have already made final, so that their composition is the exact characteristic foot
+ * and no O((q/m)|B| dt) splitting error remains. Same limiter and flux polynomial; closed velocity box;
+ * every face needs |s_face| < 1 (MPHV_ERR_RANGE otherwise). Needs all three velocity dimensions
+ * active (MPHV_ERR_ARG otherwise). It applies to mphv_sweep_v (call dims 0, 1, 2 in that order with the
+ * same dt), mphv_stage_v, mphv_step, mphv_step_moments and mphv_run_host. The face coefficients depend
+ * on (fields, dt): the first call with a new dt after mphv_set_fields or mphv_set_vmode runs one small
+ * kernel and synchronises the stream once; later calls with the same dt only enqueue. */
+enum { MPHV_V_PLAIN = 0, MPHV_V_BACKSUB = 1 };
+int mphv_set_vmode(mphv_ctx *ctx, int mode);
+
 /* Tuning knob for experiments and tests. level 0 = one kernel per sweep; 1 = pairwise fused
  * kernels (V_vx+V_vy per velocity plane, V_vz+moments; the default, fastest measured on B200);
  * 2 = the whole V stage (three sweeps and the moments) in one pass over f; 3 = level 2 plus the

@@ -7,6 +7,7 @@
 #include "mphv_march.cuh"
 #include "mphv_vstage.cuh"
 #include "mphv_sxy.cuh"
+#include "mphv_backsub.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -35,6 +36,9 @@ struct mphv_ctx {
     int vs_T, vs_grid, vs_variant; size_t vs_smem;   // second-generation whole-V-stage kernel (T = 0: unsupported)
     int sxy_T, sxy_C; size_t sxy_smem;               // fused S_x + S_y kernel (T = 0: unsupported)
     int cube_T, cube_grid, cube_variant, plane_grid; size_t cube_smem, plane_smem;  // whole-V-stage cube kernel launch shape (T = 0: unsupported)
+    int vmode;                                       // 0 plain V sweeps, 1 backsubstitution
+    double *bs_K;                                    // device [ns][12] face-displacement coefficients + [3] maxima
+    double bs_dt; bool bs_valid; double bs_smax[3];
     uint64_t launches;
     int fusion;
     int timing;
@@ -47,11 +51,11 @@ struct mphv_ctx {
 };
 
 enum { SLOT_SX0 = 0, SLOT_SX1, SLOT_SX2, SLOT_VX, SLOT_VY, SLOT_VZ, SLOT_MOM, SLOT_VXY, SLOT_VZMOM,
-       SLOT_SHIFT, SLOT_SUM, SLOT_AMAX, SLOT_VCUBE, SLOT_VCUBE_MOM, SLOT_PACK, SLOT_SXY, SLOT_COUNT };
+       SLOT_SHIFT, SLOT_SUM, SLOT_AMAX, SLOT_VCUBE, SLOT_VCUBE_MOM, SLOT_PACK, SLOT_SXY, SLOT_BSCOEF, SLOT_COUNT };
 static const char *const SLOT_NAMES[SLOT_COUNT] = {
     "sweep_x0", "sweep_x1", "sweep_x2", "sweep_vx", "sweep_vy", "sweep_vz", "moments",
     "fused_vx_vy", "fused_vz_moments", "shift_periodic", "sum_f", "amax_fields",
-    "fused_vx_vy_vz", "fused_vx_vy_vz_moments", "pack_halo", "fused_sx_sy" };
+    "fused_vx_vy_vz", "fused_vx_vy_vz_moments", "pack_halo", "fused_sx_sy", "backsub_coefficients" };
 
 namespace {
 
@@ -382,8 +386,57 @@ int do_sweep_x(mphv_ctx *c, int d, double dt)
     return MPHV_OK;
 }
 
+// ---- backsubstitution mode (mphv_backsub.cuh) ---------------------------------------------
+// Coefficients and max |s_face| depend on (fields, dt): evaluated on the first use of a new dt
+// (one kernel, 3 doubles to the host, one stream synchronisation), then cached.
+int ensure_backsub(mphv_ctx *c, double dt)
+{
+    if (c->bs_valid && c->bs_dt == dt) return MPHV_OK;
+    unsigned long long *smax = reinterpret_cast<unsigned long long *>(c->bs_K + 12 * c->ns);
+    CUDA_TRY(c, cudaMemsetAsync(smax, 0, 3 * sizeof(unsigned long long), c->stream));
+    int st;
+    {
+        Timed tm(c, SLOT_BSCOEF, 0.0);
+        backsub_coeff_kernel<<<grid_for((long long)c->ns, 128), 128, 0, c->stream>>>(c->E, c->B, c->gd, dt, c->bs_K, smax);
+        st = after_launch(c, "backsub_coeff_kernel");
+    }
+    if (st != MPHV_OK) return st;
+    CUDA_TRY(c, cudaMemcpyAsync(c->bs_smax, smax, 3 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    c->bs_dt = dt; c->bs_valid = true;
+    return MPHV_OK;
+}
+
+int do_sweep_v_backsub(mphv_ctx *c, int d)
+{
+    BacksubArgs a;
+    a.f = c->f; a.K = c->bs_K; a.g = c->gd;
+    const long long nvx = c->grid.nv[0], nvy = c->grid.nv[1], nvz = c->grid.nv[2];
+    Timed tm(c, SLOT_VX + d, 16.0 * (double)c->nf);
+    if (d == 0) {
+        const long long rows = (long long)c->ns * nvz * nvy;
+        const int block = 256;
+        const int ch = (nvx % 4 == 0) ? 4 : (nvx % 2 == 0 ? 2 : 1);
+        const int cpr = (int)(nvx / ch);
+        if (cpr > block) { set_err(c, "nvx = %lld too large for the vx kernel (max %d)", nvx, block * 4); return MPHV_ERR_ARG; }
+        const int rpc = block / cpr;
+        const unsigned grid = (unsigned)((rows + rpc - 1) / rpc);
+        if (ch == 4)      bs_vx_kernel<4><<<grid, block, 0, c->stream>>>(a, rows, rpc);
+        else if (ch == 2) bs_vx_kernel<2><<<grid, block, 0, c->stream>>>(a, rows, rpc);
+        else              bs_vx_kernel<1><<<grid, block, 0, c->stream>>>(a, rows, rpc);
+        return after_launch(c, "bs_vx_kernel");
+    }
+    const long long outer = d == 2 ? (long long)c->ns : (long long)c->ns * nvz;
+    const long long inner = d == 2 ? nvy * nvx : nvx;
+    const int n = c->grid.nv[d];
+    if (inner % 2 == 0) bs_march_kernel<2, 4><<<grid_for(outer * (inner / 2), 256), 256, 0, c->stream>>>(a, d, outer, n, inner);
+    else                bs_march_kernel<1, 4><<<grid_for(outer * inner, 256), 256, 0, c->stream>>>(a, d, outer, n, inner);
+    return after_launch(c, "bs_march_kernel");
+}
+
 int do_sweep_v(mphv_ctx *c, int d, double dt)
 {
+    if (c->vmode) return do_sweep_v_backsub(c, d);
     if (d == 0) {
         VxArgs a;
         std::memset(&a, 0, sizeof a);
@@ -417,6 +470,11 @@ int do_v_stage(mphv_ctx *c, double dt, double *n, double *j, double *P)
 {
     int st;
     const bool ax = c->grid.nv[0] > 1, ay = c->grid.nv[1] > 1, az = c->grid.nv[2] > 1;
+    if (c->vmode) {                                  // backsubstitution: three face-displaced sweeps, then the moments
+        for (int d = 0; d < 3; ++d)
+            if ((st = do_sweep_v_backsub(c, d)) != MPHV_OK) return st;
+        return n ? do_moments(c, n, j, P) : MPHV_OK;
+    }
     if (c->fusion >= 2 && c->vs_T > 0) return launch_vstage(c, dt, n, j, P);
     if (c->fusion >= 2 && c->cube_T > 0) return launch_vcube(c, dt, true, n, j, P);
     if (c->fusion && c->cube_T > 0 && c->plane_grid > 0) {
@@ -470,6 +528,15 @@ int range_x(mphv_ctx *c, int d, double dt)
 
 int range_v(mphv_ctx *c, int d, double dt)
 {
+    if (c->vmode) {
+        int st = ensure_backsub(c, dt);
+        if (st != MPHV_OK) return st;
+        if (!(c->bs_smax[d] < 1.0)) {
+            set_err(c, "backsubstituted velocity sweep %d: max |s_face| = %g >= 1 (closed velocity box)", d, c->bs_smax[d]);
+            return MPHV_ERR_RANGE;
+        }
+        return MPHV_OK;
+    }
     const double smax = max_courant_v(c, d, dt);
     if (!(smax < 1.0)) { set_err(c, "velocity sweep %d: max |s| = %g >= 1 (closed velocity box)", d, smax); return MPHV_ERR_RANGE; }
     return MPHV_OK;
@@ -637,6 +704,7 @@ int mphv_destroy(mphv_ctx *c)
 {
     if (!c) return MPHV_ERR_ARG;
     if (c->ws) cudaFree(c->ws);
+    if (c->bs_K) cudaFree(c->bs_K);
     if (c->pending) { drain_timing(c, false); delete c->pending; }
     delete c;
     return MPHV_OK;
@@ -678,6 +746,7 @@ int mphv_set_fields(mphv_ctx *c, const double *E, const double *B)
     CUDA_TRY(c, cudaMemcpyAsync(h, out, sizeof h, cudaMemcpyDeviceToHost, c->stream));
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     c->E = E; c->B = B;
+    c->bs_valid = false;
     for (int d = 0; d < 3; ++d) c->amax[d] = h[d];
     return MPHV_OK;
 }
@@ -870,6 +939,24 @@ int mphv_get_timing(mphv_ctx *c, int slot, char *name, size_t name_cap, double *
 }
 
 uint64_t mphv_launch_count(const mphv_ctx *c) { return c ? c->launches : 0; }
+
+int mphv_set_vmode(mphv_ctx *c, int mode)
+{
+    if (!c) return MPHV_ERR_ARG;
+    if (mode != MPHV_V_PLAIN && mode != MPHV_V_BACKSUB) { set_err(c, "vmode must be MPHV_V_PLAIN or MPHV_V_BACKSUB"); return MPHV_ERR_ARG; }
+    if (mode == MPHV_V_BACKSUB) {
+        if (c->grid.nv[0] < 2 || c->grid.nv[1] < 2 || c->grid.nv[2] < 2) {
+            set_err(c, "backsubstitution needs all three velocity dimensions active"); return MPHV_ERR_ARG;
+        }
+        if (!c->bs_K) {
+            cudaError_t e = cudaMalloc(&c->bs_K, (12 * c->ns + 4) * sizeof(double));
+            if (e != cudaSuccess) { c->bs_K = nullptr; return cuda_fail(c, e, "cudaMalloc backsubstitution coefficients"); }
+        }
+    }
+    c->vmode = mode;
+    c->bs_valid = false;
+    return MPHV_OK;
+}
 
 int mphv_set_fusion(mphv_ctx *c, int enabled)
 {

@@ -25,7 +25,7 @@ SYMBOLS = (
     "mphv_create", "mphv_destroy", "mphv_set_stream", "mphv_f_count", "mphv_space_count",
     "mphv_bind_f", "mphv_set_fields", "mphv_sweep_x", "mphv_sweep_v", "mphv_step",
     "mphv_moments", "mphv_step_moments", "mphv_run_host", "mphv_sum_f", "mphv_launch_count",
-    "mphv_set_fusion", "mphv_strerror", "mphv_last_error",
+    "mphv_set_fusion", "mphv_set_vmode", "mphv_strerror", "mphv_last_error",
     "mphv_set_timing", "mphv_timing_slots", "mphv_get_timing",
     "mphv_stage_x", "mphv_stage_v", "mphv_halo_count", "mphv_pack_halo", "mphv_sweep_x_halo",
 )
@@ -75,6 +75,7 @@ def lib() -> C.CDLL:
         "mphv_sum_f": (i32, [vp, vp]),
         "mphv_launch_count": (C.c_uint64, [vp]),
         "mphv_set_fusion": (i32, [vp, i32]),
+        "mphv_set_vmode": (i32, [vp, i32]),
         "mphv_set_timing": (i32, [vp, i32]),
         "mphv_timing_slots": (i32, []),
         "mphv_get_timing": (i32, [vp, i32, C.c_char_p, C.c_size_t, C.POINTER(dbl),
@@ -199,6 +200,13 @@ def mphv_sum_f(ctx, sum_dev: int):
 
 def mphv_launch_count(ctx) -> int:
     return int(lib().mphv_launch_count(ctx))
+
+
+V_PLAIN, V_BACKSUB = 0, 1
+
+
+def mphv_set_vmode(ctx, mode):
+    _check(ctx, lib().mphv_set_vmode(ctx, int(mode)))
 
 
 def mphv_set_fusion(ctx, level):
@@ -339,6 +347,9 @@ class Vlasov:
     @property
     def launches(self) -> int:
         return mphv_launch_count(self.ctx)
+
+    def set_vmode(self, mode):
+        mphv_set_vmode(self.ctx, mode)
 
     def set_fusion(self, level):
         mphv_set_fusion(self.ctx, level)
