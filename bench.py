@@ -43,8 +43,10 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs index (default 3, headline)")
     ap.add_argument("--impl", default="mphv", choices=["mphv", "reference"])
-    ap.add_argument("--fusion", type=int, default=1, choices=[0, 1, 2, 3],
-                    help="mphv_set_fusion level: 0 one kernel per sweep, 1 pairwise fused, 2 whole V stage in one kernel, 3 also S_x+S_y in one kernel; default 1")
+    ap.add_argument("--fusion", type=int, default=3, choices=[0, 1, 2, 3],
+                    help="mphv_set_fusion level: 0 one kernel per sweep, 1 pairwise fused, 2 whole V stage in one kernel, 3 also S_x+S_y in one kernel; default 3")
+    ap.add_argument("--vmode", default="plain", choices=["plain", "backsub"],
+                    help="V stage: plain 1-D sweeps (BASELINE.json north_star, default) or backsubstitution (P:L137)")
     ap.add_argument("--decomp", default="auto", choices=["auto", "halo", "none"],
                     help="'halo' = one spatially decomposed problem with neighbour exchange (the default for N > 1; "
                          "at N = 1 the block is its own periodic neighbour), 'none' = N independent problems "
@@ -233,6 +235,8 @@ def run_mphv(args, w):
         sim = mphv.Vlasov.from_workload(wr, device=dev)
         step_moments = sim.step_moments
     sim.set_fusion(args.fusion)
+    if args.vmode == "backsub":
+        sim.set_vmode(mphv.V_BACKSUB)
     f = torch.from_numpy(f0).to(dev)
     sim.bind_f(f)
     sim.set_fields(torch.from_numpy(E).to(dev), torch.from_numpy(B).to(dev))
@@ -302,7 +306,7 @@ def run_mphv(args, w):
         "config": {"workload": w.name, "cells_per_gpu": w.n_cells, "bytes_per_copy_of_f": w.n_cells * 8,
                    "step": "S_x,S_y[,S_z],V_vx,V_vy,V_vz + moments n,j,P every step",
                    "l2": "inputs larger than L2 (f is %.2f GB >> 126 MB); no flush needed" % (w.n_cells * 8 / 1e9),
-                   "fusion": args.fusion,
+                   "fusion": args.fusion, "vmode": args.vmode,
                    "parallelism": "1 GPU" if world == 1 else
                    (f"{world} spatial blocks along periodic x, 2-layer halo exchange before S_x (NCCL send/recv), "
                     f"{2 * sim.halo_count(0) * 8} B sent per rank per step" if halo_mode else f"{world} independent problems")},

@@ -192,9 +192,9 @@ enum { MPHV_V_PLAIN = 0, MPHV_V_BACKSUB = 1 };
 int mphv_set_vmode(mphv_ctx *ctx, int mode);
 
 /* Tuning knob for experiments and tests. level 0 = one kernel per sweep; 1 = pairwise fused
- * kernels (V_vx+V_vy per velocity plane, V_vz+moments; the default, fastest measured on B200);
+ * kernels (V_vx+V_vy per velocity plane, V_vz+moments);
  * 2 = the whole V stage (three sweeps and the moments) in one pass over f; 3 = level 2 plus the
- * spatial sweeps S_x and S_y in one pass over f. Levels 1..3 fall back to lower-level kernels for
+ * spatial sweeps S_x and S_y in one pass over f (the default, fastest measured on B200). Levels 1..3 fall back to lower-level kernels for
  * grids their kernels do not cover (nvx, nvy not multiples of 4 resp. 2, fewer than 3 velocity
  * dimensions; nx not a multiple of 4, nvel not a multiple of 8, |s| >= 1 on a periodic axis).
  * Results agree up to fp64 rounding at every level. */

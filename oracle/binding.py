@@ -112,6 +112,10 @@ def lib() -> C.CDLL:
         L.orc_sweep_v_backsub.restype = C.c_int
         L.orc_step_backsub.argtypes = L.orc_step.argtypes
         L.orc_step_backsub.restype = C.c_int
+        L.orc_maxwellian.argtypes = [C.POINTER(_CGrid), C.POINTER(_CBox), C.c_size_t, dp, dp, dp, dp]
+        L.orc_maxwellian.restype = C.c_int
+        L.orc_exchange_maxwellian.argtypes = [dp, C.POINTER(_CGrid), C.POINTER(_CBox), C.c_int, C.c_int, dp, dp, dp]
+        L.orc_exchange_maxwellian.restype = C.c_int
         L.orc_num_threads.argtypes = []
         L.orc_num_threads.restype = C.c_int
         _lib = L
@@ -234,6 +238,33 @@ def moments(f: np.ndarray, grid: Grid, box: Box):
     if st != OK:
         raise ValueError(f"orc_moments status {st}")
     return n, j, P
+
+
+def maxwellian(grid: Grid, box: Box, n, j, P) -> np.ndarray:
+    """Ten-moment Maxwellian cubes of `count` cells: n [count], j [3][count], P [6][count] -> [count][nvz][nvy][nvx]."""
+    n = np.ascontiguousarray(n, dtype=np.float64).reshape(-1)
+    count = n.size
+    j = np.ascontiguousarray(j, dtype=np.float64).reshape(3, count)
+    P = np.ascontiguousarray(P, dtype=np.float64).reshape(6, count)
+    out = np.empty((count, grid.nv[2], grid.nv[1], grid.nv[0]))
+    g, b = grid.c(), box.c()
+    st = lib().orc_maxwellian(C.byref(g), C.byref(b), count, _p(n), _p(j), _p(P), _p(out))
+    if st != OK:
+        raise ValueError(f"orc_maxwellian status {st}")
+    return out
+
+
+def exchange_maxwellian(f: np.ndarray, grid: Grid, box: Box, dim: int, side: int, n_fl, j_fl, P_fl) -> None:
+    """Exchange of Maxwellians in the two boundary layers at one end of spatial axis dim, in place."""
+    _check_f(f, grid)
+    plane = grid.n_space // grid.nx[dim]
+    n_fl = np.ascontiguousarray(n_fl, dtype=np.float64); assert n_fl.size == 2 * plane
+    j_fl = np.ascontiguousarray(j_fl, dtype=np.float64); assert j_fl.size == 6 * plane
+    P_fl = np.ascontiguousarray(P_fl, dtype=np.float64); assert P_fl.size == 12 * plane
+    g, b = grid.c(), box.c()
+    st = lib().orc_exchange_maxwellian(_p(f), C.byref(g), C.byref(b), int(dim), int(side), _p(n_fl), _p(j_fl), _p(P_fl))
+    if st != OK:
+        raise ValueError(f"orc_exchange_maxwellian status {st}")
 
 
 def total(f: np.ndarray) -> float:

@@ -27,7 +27,9 @@
  * conservation, positivity, mirror symmetry, free streaming, gyration closure,
  * uniform-E shift, Maxwellian and hand-summed moments; for the backsubstituted V
  * stage (R15): exact-rational composition of the three foot maps, reduction to the
- * plain sweeps at B = 0, gyration closure at large angle, conservation, positivity.
+ * plain sweeps at B = 0, gyration closure at large angle, conservation, positivity;
+ * for the ten-moment Maxwellian and the exchange of Maxwellians (R16, R17): closed
+ * form, scipy's multivariate normal, moment reproduction, the sigma weights.
  * PARITY UNPINNED against the authors' own implementation: PAPER.md prints no
  * value of their scheme's output anywhere.
  *
@@ -595,6 +597,176 @@ int orc_step_backsub(double *f, const orc_grid *g, const orc_box *b, double q_ov
         if (st != ORC_OK) return st;
     }
     if (net_out) *net_out = net;
+    return ORC_OK;
+}
+
+/* ==========================================================================
+ * Ten-moment Maxwellian and the "exchange of Maxwellians" at a Vlasov / ten-moment
+ * coupling border.
+ * P:L185 (sec. 4.3): "The first guess is to use a ten-moment Maxwellian distribution,
+ * which takes the temperature tensor into account (a multivariate normal
+ * distribution), as this is the maximum entropy solution."
+ * "we extend the Vlasov data at the coupling border into the boundary cells
+ * and adjust it to match the fluid boundary data ... by exchanging Maxwellians. We
+ * remove the ten-moment Maxwellian part from the extended Vlasov data and add the
+ * result, multiplied by a factor sigma_i, to the Maxwellian computed from the fluid
+ * boundary data. The factor is chosen to decrease linearly with distance to the
+ * coupling border. In our case of two boundary cells, it is sigma_1 = 2/3 and
+ * sigma_2 = 1/3 in the first and second boundary cells, respectively."
+ *
+ * Readings (R16, R17): with the moment conventions of c-8 (n = int f,
+ * j = int v f, P = int v v f: full second moment, no mass factor)
+ *   u = j / n,  C_ab = P_ab / n - u_a u_b   (covariance = temperature tensor / m),
+ *   M[n,j,P](v) = n (2 pi)^(-D/2) det(C)^(-1/2) exp(-(v-u)^T C^-1 (v-u) / 2)
+ * over the D active velocity dimensions, evaluated at the velocity cell centres
+ * (the point values the midpoint quadrature of c-8 integrates). n <= 0 or C not
+ * positive definite: M = 0. "Extend the Vlasov data into the boundary cells" =
+ * zero-gradient copy of the last interior cell along the axis (the paper states no
+ * extrapolation rule).
+ * ========================================================================== */
+
+/* covariance inverse and normalisation of one cell; returns 0 if degenerate. Only the active
+ * velocity dimensions enter (an inactive one has a single cell at v = 0 with dv = 1). */
+static int maxwellian_setup(const orc_grid *g, double n, const double j[3], const double P[6],
+                            double u[3], double Ci[3][3], double *norm)
+{
+    if (!(n > 0.0)) return 0;
+    int act[3], D = 0;
+    for (int d = 0; d < 3; ++d) if (g->nv[d] > 1) act[D++] = d;
+    static const int pidx[3][3] = { { 0, 1, 2 }, { 1, 3, 4 }, { 2, 4, 5 } };
+    double C[3][3];
+    for (int a = 0; a < 3; ++a) u[a] = j[a] / n;
+    for (int a = 0; a < D; ++a)
+        for (int b = 0; b < D; ++b)
+            C[a][b] = P[pidx[act[a]][act[b]]] / n - u[act[a]] * u[act[b]];
+    double det;
+    double inv[3][3] = { { 0 } };
+    if (D == 1) { det = C[0][0]; if (!(det > 0.0)) return 0; inv[0][0] = 1.0 / det; }
+    else if (D == 2) {
+        det = C[0][0] * C[1][1] - C[0][1] * C[1][0];
+        if (!(C[0][0] > 0.0) || !(det > 0.0)) return 0;
+        inv[0][0] = C[1][1] / det; inv[1][1] = C[0][0] / det; inv[0][1] = inv[1][0] = -C[0][1] / det;
+    } else if (D == 3) {
+        double c00 = C[1][1] * C[2][2] - C[1][2] * C[2][1];
+        double c01 = C[1][2] * C[2][0] - C[1][0] * C[2][2];
+        double c02 = C[1][0] * C[2][1] - C[1][1] * C[2][0];
+        det = C[0][0] * c00 + C[0][1] * c01 + C[0][2] * c02;
+        double m2 = C[0][0] * C[1][1] - C[0][1] * C[1][0];
+        if (!(C[0][0] > 0.0) || !(m2 > 0.0) || !(det > 0.0)) return 0;     /* Sylvester */
+        inv[0][0] = c00 / det; inv[0][1] = (C[0][2] * C[2][1] - C[0][1] * C[2][2]) / det;
+        inv[0][2] = (C[0][1] * C[1][2] - C[0][2] * C[1][1]) / det;
+        inv[1][0] = c01 / det; inv[1][1] = (C[0][0] * C[2][2] - C[0][2] * C[2][0]) / det;
+        inv[1][2] = (C[0][2] * C[1][0] - C[0][0] * C[1][2]) / det;
+        inv[2][0] = c02 / det; inv[2][1] = (C[0][1] * C[2][0] - C[0][0] * C[2][1]) / det;
+        inv[2][2] = m2 / det;
+    } else return 0;
+    for (int a = 0; a < 3; ++a) for (int b = 0; b < 3; ++b) Ci[a][b] = 0.0;
+    for (int a = 0; a < D; ++a) for (int b = 0; b < D; ++b) Ci[act[a]][act[b]] = inv[a][b];
+    const double two_pi = 6.283185307179586476925286766559;
+    *norm = n / (pow(two_pi, 0.5 * D) * sqrt(det));
+    return 1;
+}
+
+/* one velocity cube [nvz][nvy][nvx] of M[n, j, P] */
+static void maxwellian_cube(const orc_grid *g, const orc_box *b, double n, const double j[3],
+                            const double P[6], double *cube)
+{
+    double u[3], Ci[3][3], norm;
+    const int ok = maxwellian_setup(g, n, j, P, u, Ci, &norm);
+    for (int jz = 0; jz < g->nv[2]; ++jz)
+        for (int jy = 0; jy < g->nv[1]; ++jy)
+            for (int jx = 0; jx < g->nv[0]; ++jx) {
+                double val = 0.0;
+                if (ok) {
+                    double d[3] = { v_centre(g, b, 0, jx) - u[0], v_centre(g, b, 1, jy) - u[1], v_centre(g, b, 2, jz) - u[2] };
+                    double q = 0.0;
+                    for (int a = 0; a < 3; ++a) for (int c = 0; c < 3; ++c) q += Ci[a][c] * d[a] * d[c];
+                    val = norm * exp(-0.5 * q);
+                }
+                cube[((size_t)jz * g->nv[1] + jy) * g->nv[0] + jx] = val;
+            }
+}
+
+/* f_out[count][nvel] = M[n[c], j[.][c], P[.][c]] for c < count (arrays n[count], j[3][count], P[6][count]) */
+int orc_maxwellian(const orc_grid *g, const orc_box *b, size_t count, const double *n,
+                   const double *j, const double *P, double *f_out)
+{
+    if (!grid_ok(g, b) || !n || !j || !P || !f_out) return ORC_ERR_ARG;
+    const size_t nvel = n_vel(g);
+    for (size_t c = 0; c < count; ++c) {
+        double jc[3] = { j[c], j[count + c], j[2 * count + c] };
+        double Pc[6];
+        for (int a = 0; a < 6; ++a) Pc[a] = P[(size_t)a * count + c];
+        maxwellian_cube(g, b, n[c], jc, Pc, f_out + c * nvel);
+    }
+    return ORC_OK;
+}
+
+/* moments of one cube by the midpoint rule (c-8), plain double accumulation in long double */
+static void cube_moments(const orc_grid *g, const orc_box *b, const double *cube, double *n, double j[3], double P[6])
+{
+    const long double dV = (long double)v_width(g, b, 0) * v_width(g, b, 1) * v_width(g, b, 2);
+    long double m0 = 0, m1[3] = { 0, 0, 0 }, m2[6] = { 0, 0, 0, 0, 0, 0 };
+    for (int jz = 0; jz < g->nv[2]; ++jz)
+        for (int jy = 0; jy < g->nv[1]; ++jy)
+            for (int jx = 0; jx < g->nv[0]; ++jx) {
+                long double fv = cube[((size_t)jz * g->nv[1] + jy) * g->nv[0] + jx];
+                long double vx = v_centre(g, b, 0, jx), vy = v_centre(g, b, 1, jy), vz = v_centre(g, b, 2, jz);
+                m0 += fv;
+                m1[0] += vx * fv; m1[1] += vy * fv; m1[2] += vz * fv;
+                m2[0] += vx * vx * fv; m2[1] += vx * vy * fv; m2[2] += vx * vz * fv;
+                m2[3] += vy * vy * fv; m2[4] += vy * vz * fv; m2[5] += vz * vz * fv;
+            }
+    *n = (double)(m0 * dV);
+    for (int a = 0; a < 3; ++a) j[a] = (double)(m1[a] * dV);
+    for (int a = 0; a < 6; ++a) P[a] = (double)(m2[a] * dV);
+}
+
+/*
+ * Exchange of Maxwellians at one end of spatial axis dim (side 0: low end, 1: high end) of the
+ * block f: the two outermost cell layers are the boundary cells. For every column along dim,
+ *   f_ext   = cube of the last interior cell (layer 2 from the end), copied into both boundary cells,
+ *   ghost_i = M[fluid data of boundary cell i] + sigma_i (f_ext - M[moments of f_ext]),
+ * sigma = 2/3 in the boundary cell next to the interior, 1/3 in the outer one.
+ * n_fl [2][plane], j_fl [3][2][plane], P_fl [6][2][plane]: layer 0 = lower spatial index; plane =
+ * the other two spatial indices in C order (z slower than y slower than x).
+ */
+int orc_exchange_maxwellian(double *f, const orc_grid *g, const orc_box *b, int dim, int side,
+                            const double *n_fl, const double *j_fl, const double *P_fl)
+{
+    if (!f || !grid_ok(g, b) || dim < 0 || dim > 2 || (side != 0 && side != 1)) return ORC_ERR_ARG;
+    if (!n_fl || !j_fl || !P_fl || g->nx[dim] < 4) return ORC_ERR_ARG;
+    const size_t nvel = n_vel(g);
+    const int n = g->nx[dim];
+    size_t sstride[3] = { 1, (size_t)g->nx[0], (size_t)g->nx[0] * g->nx[1] };     /* in spatial cells */
+    const int da = dim == 0 ? 1 : 0, db = dim == 2 ? 1 : 2;                        /* da faster than db */
+    const size_t plane = (size_t)g->nx[da] * g->nx[db];
+    double *Mfl = (double *)malloc(nvel * sizeof(double));
+    double *Mex = (double *)malloc(nvel * sizeof(double));
+    if (!Mfl || !Mex) { free(Mfl); free(Mex); return ORC_ERR_ARG; }
+    for (int ib = 0; ib < g->nx[db]; ++ib)
+        for (int ia = 0; ia < g->nx[da]; ++ia) {
+            const size_t pl = (size_t)ib * g->nx[da] + ia;
+            const size_t col = (size_t)ia * sstride[da] + (size_t)ib * sstride[db];
+            const int interior = side ? n - 3 : 2;
+            const double *fext = f + (col + (size_t)interior * sstride[dim]) * nvel;
+            double ne, je[3], Pe[6];
+            cube_moments(g, b, fext, &ne, je, Pe);
+            maxwellian_cube(g, b, ne, je, Pe, Mex);
+            for (int layer = 0; layer < 2; ++layer) {
+                const int idx = side ? n - 2 + layer : layer;
+                const int dist = side ? layer + 1 : 2 - layer;           /* 1 = next to the interior */
+                const double sigma = dist == 1 ? 2.0 / 3.0 : 1.0 / 3.0;
+                const size_t k = (size_t)layer * plane + pl;
+                double jf[3] = { j_fl[k], j_fl[2 * plane + k], j_fl[4 * plane + k] };
+                double Pf[6];
+                for (int a = 0; a < 6; ++a) Pf[a] = P_fl[(size_t)a * 2 * plane + k];
+                maxwellian_cube(g, b, n_fl[k], jf, Pf, Mfl);
+                double *dst = f + (col + (size_t)idx * sstride[dim]) * nvel;
+                for (size_t e = 0; e < nvel; ++e) dst[e] = Mfl[e] + sigma * (fext[e] - Mex[e]);
+            }
+        }
+    free(Mfl); free(Mex);
     return ORC_OK;
 }
 

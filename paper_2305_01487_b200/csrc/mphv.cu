@@ -580,7 +580,7 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
     c->ns = (size_t)grid->nx[0] * grid->nx[1] * grid->nx[2];
     c->nvel = (size_t)grid->nv[0] * grid->nv[1] * grid->nv[2];
     c->nf = c->ns * c->nvel;
-    c->fusion = 1;
+    c->fusion = 3;
     for (int d = 0; d < 3; ++d) {
         c->dx[d] = grid->nx[d] > 1 ? (box->xhi[d] - box->xlo[d]) / (double)grid->nx[d] : 1.0;
         c->dv[d] = grid->nv[d] > 1 ? (box->vhi[d] - box->vlo[d]) / (double)grid->nv[d] : 1.0;
