@@ -176,6 +176,26 @@ int mphv_timing_slots(void);
 int mphv_get_timing(mphv_ctx *ctx, int slot, char *name, size_t name_cap, double *total_ms,
                     uint64_t *launches, double *alg_bytes_per_launch);
 
+/* ---- model coupling at a Vlasov / ten-moment border (sec. 4.3; readings R16, R17).
+ * mphv_maxwellian: f_out_dev[c][nvel] = the ten-moment Maxwellian ("a multivariate normal distribution",
+ * P:L185) of cell c < count: with u = j/n and C_ab = P_ab/n - u_a u_b (moment conventions of
+ * mphv_moments: j = int v f, P = int v v f),
+ *     M(v) = n (2 pi)^(-D/2) det(C)^(-1/2) exp(-(v-u)^T C^-1 (v-u) / 2)
+ * at the velocity cell centres, D = number of active velocity dimensions. n <= 0 or C not positive
+ * definite gives M = 0 for that cell. Layouts: n_dev [count], j_dev [3][count], P_dev [6][count]
+ * (xx, xy, xz, yy, yz, zz), f_out_dev [count][nvz][nvy][nvx]; all device memory of the caller.
+ * mphv_exchange_maxwellian: "exchanging Maxwellians" in the two boundary cells at one end
+ * (side 0 = low, 1 = high index) of spatial axis dim of the bound f, in place: for every column,
+ *     ghost_i = M[fluid data of boundary cell i] + sigma_i (f_ext - M[moments of f_ext]),
+ * f_ext = the last interior cell (third from the end; zero-gradient extension), sigma = 2/3 in the
+ * boundary cell next to the interior and 1/3 in the outer one. Fluid data n_fl_dev [2][plane],
+ * j_fl_dev [3][2][plane], P_fl_dev [6][2][plane]: layer 0 = lower index along dim, plane = the other two
+ * spatial indices in C order. Needs nx[dim] >= 4. Both calls only enqueue. */
+int mphv_maxwellian(mphv_ctx *ctx, size_t count, const double *n_dev, const double *j_dev,
+                    const double *P_dev, double *f_out_dev);
+int mphv_exchange_maxwellian(mphv_ctx *ctx, int dim, int side, const double *n_fl_dev,
+                             const double *j_fl_dev, const double *P_fl_dev);
+
 /* Mode of the V stage. MPHV_V_PLAIN (default; BASELINE.json north_star): three plain 1-D sweeps with
  * the Courant numbers a_d dt / dv_d, a = (q/m)(E + v x B) at the cell centres. MPHV_V_BACKSUB: "The
  * velocity space splitting is realized via backsubstitution" (sec. 4.1; reading R15 of

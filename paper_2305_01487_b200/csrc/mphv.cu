@@ -8,6 +8,7 @@
 #include "mphv_vstage.cuh"
 #include "mphv_sxy.cuh"
 #include "mphv_backsub.cuh"
+#include "mphv_maxwell.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -51,11 +52,11 @@ struct mphv_ctx {
 };
 
 enum { SLOT_SX0 = 0, SLOT_SX1, SLOT_SX2, SLOT_VX, SLOT_VY, SLOT_VZ, SLOT_MOM, SLOT_VXY, SLOT_VZMOM,
-       SLOT_SHIFT, SLOT_SUM, SLOT_AMAX, SLOT_VCUBE, SLOT_VCUBE_MOM, SLOT_PACK, SLOT_SXY, SLOT_BSCOEF, SLOT_COUNT };
+       SLOT_SHIFT, SLOT_SUM, SLOT_AMAX, SLOT_VCUBE, SLOT_VCUBE_MOM, SLOT_PACK, SLOT_SXY, SLOT_BSCOEF, SLOT_MAXW, SLOT_EXCH, SLOT_COUNT };
 static const char *const SLOT_NAMES[SLOT_COUNT] = {
     "sweep_x0", "sweep_x1", "sweep_x2", "sweep_vx", "sweep_vy", "sweep_vz", "moments",
     "fused_vx_vy", "fused_vz_moments", "shift_periodic", "sum_f", "amax_fields",
-    "fused_vx_vy_vz", "fused_vx_vy_vz_moments", "pack_halo", "fused_sx_sy", "backsub_coefficients" };
+    "fused_vx_vy_vz", "fused_vx_vy_vz_moments", "pack_halo", "fused_sx_sy", "backsub_coefficients", "maxwellian", "exchange_maxwellian" };
 
 namespace {
 
@@ -869,6 +870,41 @@ int mphv_sweep_x_halo(mphv_ctx *c, int dim, double dt, const double *lo, const d
     MarchArgs a = march_args_space(c, dim, dt);
     a.halo_lo = lo; a.halo_hi = hi;
     return launch_march<KIND_SPACE, BC_HALO>(c, a);
+}
+
+int mphv_maxwellian(mphv_ctx *c, size_t count, const double *n, const double *j, const double *P, double *f_out)
+{
+    if (!c) return MPHV_ERR_ARG;
+    if (!n || !j || !P || !f_out) { set_err(c, "n_dev, j_dev, P_dev or f_out_dev is NULL"); return MPHV_ERR_ARG; }
+    if (count == 0) return MPHV_OK;
+    if (count > 0x7fffffffu) { set_err(c, "count too large"); return MPHV_ERR_ARG; }
+    MaxwArgs a;
+    a.n = n; a.j = j; a.P = P; a.count = (long long)count; a.f_out = f_out; a.g = c->gd;
+    Timed tm(c, SLOT_MAXW, 8.0 * (double)count * (double)c->nvel);
+    maxwellian_kernel<<<(unsigned)count, 256, 0, c->stream>>>(a);
+    return after_launch(c, "maxwellian_kernel");
+}
+
+int mphv_exchange_maxwellian(mphv_ctx *c, int dim, int side, const double *n_fl, const double *j_fl, const double *P_fl)
+{
+    if (!c) return MPHV_ERR_ARG;
+    if (dim < 0 || dim > 2 || c->grid.nx[dim] < 4) { set_err(c, "spatial dim %d out of range or inactive", dim); return MPHV_ERR_ARG; }
+    if (side != 0 && side != 1) { set_err(c, "side must be 0 (low end) or 1 (high end)"); return MPHV_ERR_ARG; }
+    if (!n_fl || !j_fl || !P_fl) { set_err(c, "n_fl_dev, j_fl_dev or P_fl_dev is NULL"); return MPHV_ERR_ARG; }
+    if (!c->f) { set_err(c, "f not bound (mphv_bind_f)"); return MPHV_ERR_STATE; }
+    const long long sstride[3] = { 1, c->grid.nx[0], (long long)c->grid.nx[0] * c->grid.nx[1] };
+    const int da = dim == 0 ? 1 : 0, db = dim == 2 ? 1 : 2;
+    ExchArgs a;
+    a.f = c->f; a.n_fl = n_fl; a.j_fl = j_fl; a.P_fl = P_fl;
+    a.plane = (long long)(c->ns / (size_t)c->grid.nx[dim]);
+    a.sa = sstride[da]; a.sb = sstride[db]; a.sd = sstride[dim];
+    a.na = c->grid.nx[da]; a.n = c->grid.nx[dim]; a.side = side; a.g = c->gd;
+    const long long plane_v = (long long)c->grid.nv[0] * c->grid.nv[1];
+    int block = 512;
+    while (block > 32 && block / 2 >= plane_v) block /= 2;
+    Timed tm(c, SLOT_EXCH, 2.0 * (double)a.plane * 16.0 * (double)c->nvel);
+    exchange_kernel<<<(unsigned)(2 * a.plane), block, 0, c->stream>>>(a);
+    return after_launch(c, "exchange_kernel");
 }
 
 int mphv_step_moments(mphv_ctx *c, double dt, double *n, double *j, double *P)

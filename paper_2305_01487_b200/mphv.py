@@ -25,7 +25,7 @@ SYMBOLS = (
     "mphv_create", "mphv_destroy", "mphv_set_stream", "mphv_f_count", "mphv_space_count",
     "mphv_bind_f", "mphv_set_fields", "mphv_sweep_x", "mphv_sweep_v", "mphv_step",
     "mphv_moments", "mphv_step_moments", "mphv_run_host", "mphv_sum_f", "mphv_launch_count",
-    "mphv_set_fusion", "mphv_set_vmode", "mphv_strerror", "mphv_last_error",
+    "mphv_set_fusion", "mphv_set_vmode", "mphv_maxwellian", "mphv_exchange_maxwellian", "mphv_strerror", "mphv_last_error",
     "mphv_set_timing", "mphv_timing_slots", "mphv_get_timing",
     "mphv_stage_x", "mphv_stage_v", "mphv_halo_count", "mphv_pack_halo", "mphv_sweep_x_halo",
 )
@@ -76,6 +76,8 @@ def lib() -> C.CDLL:
         "mphv_launch_count": (C.c_uint64, [vp]),
         "mphv_set_fusion": (i32, [vp, i32]),
         "mphv_set_vmode": (i32, [vp, i32]),
+        "mphv_maxwellian": (i32, [vp, C.c_size_t, vp, vp, vp, vp]),
+        "mphv_exchange_maxwellian": (i32, [vp, i32, i32, vp, vp, vp]),
         "mphv_set_timing": (i32, [vp, i32]),
         "mphv_timing_slots": (i32, []),
         "mphv_get_timing": (i32, [vp, i32, C.c_char_p, C.c_size_t, C.POINTER(dbl),
@@ -203,6 +205,14 @@ def mphv_launch_count(ctx) -> int:
 
 
 V_PLAIN, V_BACKSUB = 0, 1
+
+
+def mphv_maxwellian(ctx, count: int, n_dev, j_dev, P_dev, f_out_dev):
+    _check(ctx, lib().mphv_maxwellian(ctx, int(count), n_dev, j_dev, P_dev, f_out_dev))
+
+
+def mphv_exchange_maxwellian(ctx, dim: int, side: int, n_fl_dev, j_fl_dev, P_fl_dev):
+    _check(ctx, lib().mphv_exchange_maxwellian(ctx, int(dim), int(side), n_fl_dev, j_fl_dev, P_fl_dev))
 
 
 def mphv_set_vmode(ctx, mode):
@@ -347,6 +357,18 @@ class Vlasov:
     @property
     def launches(self) -> int:
         return mphv_launch_count(self.ctx)
+
+    def maxwellian(self, n, j, P, out=None):
+        """Ten-moment Maxwellian cubes of n.numel() cells (device tensors n [count], j [3][count], P [6][count])."""
+        import torch
+        count = n.numel()
+        if out is None:
+            out = torch.empty((count, self.nv[2], self.nv[1], self.nv[0]), dtype=torch.float64, device=n.device)
+        mphv_maxwellian(self.ctx, count, n.data_ptr(), j.data_ptr(), P.data_ptr(), out.data_ptr())
+        return out
+
+    def exchange_maxwellian(self, dim, side, n_fl, j_fl, P_fl):
+        mphv_exchange_maxwellian(self.ctx, dim, side, n_fl.data_ptr(), j_fl.data_ptr(), P_fl.data_ptr())
 
     def set_vmode(self, mode):
         mphv_set_vmode(self.ctx, mode)

@@ -96,7 +96,7 @@ def test_distributed_vlasov_single_rank_through_the_halo_kernels(orc):
     for _ in range(2):
         orc.step(ref, grid, box, w.q_over_m, E, B, dt)
     assert rel_err(f.cpu().numpy(), ref, 3) <= 2 * TOL_SWEEP
-    assert dv.sim.launches >= 2 * (2 * 3 + 2), "pack x2 + halo sweep per spatial axis, V stage"
+    assert dv.sim.launches >= 2 * (2 * 3 + 1), "pack x2 + halo sweep per spatial axis, V stage (one kernel at the default fusion level)"
 
 
 def test_halo_api_errors():

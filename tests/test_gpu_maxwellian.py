@@ -1,0 +1,82 @@
+"""GPU parity of mphv_maxwellian and mphv_exchange_maxwellian (readings R16, R17) against
+the oracle, element by element, through the C ABI. Tolerance: |gpu - oracle| <=
+1e-12 max|cube|: the value is norm * exp(q) with q a quadratic form from a 3x3 solve, so a relative
+perturbation eps of the inverse covariance changes f by f |q| eps <= (2/e) max f * kappa * eps."""
+import numpy as np
+import pytest
+
+from test_gpu_parity import small_workload, torch_cuda, mphv  # noqa: F401
+from test_oracle_maxwellian import _moments_from
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-12
+
+
+def _random_moments(rng, count):
+    n, j, P = [], [], []
+    for _ in range(count):
+        A = 0.4 * rng.standard_normal((3, 3))
+        C = A @ A.T + np.diag(0.6 + 0.6 * rng.random(3))
+        a, b, c = _moments_from(0.3 + rng.random(), 0.8 * rng.standard_normal(3), C)
+        n.append(a); j.append(b); P.append(c)
+    return np.array(n), np.array(j).T.copy(), np.array(P).T.copy()
+
+
+@pytest.mark.parametrize("nv", [(12, 10, 8), (9, 7, 5), (40, 40, 8), (16, 12, 1), (16, 1, 1)])
+def test_maxwellian_matches_oracle(torch_cuda, mphv, orc, nv):
+    torch = torch_cuda
+    w = small_workload((4, 4, 1), nv)
+    sim = mphv.Vlasov.from_workload(w)
+    grid, box = orc.Grid(w.nx, w.nv, w.bc), orc.Box(w.xlo, w.xhi, w.vlo, w.vhi)
+    rng = np.random.default_rng(31)
+    n, j, P = _random_moments(rng, 7)
+    n[2] = 0.0                      # degenerate cells give 0
+    P[3, 4] = -1.0
+    ref = orc.maxwellian(grid, box, n, j, P)
+    out = sim.maxwellian(torch.from_numpy(n).cuda(), torch.from_numpy(j).cuda(), torch.from_numpy(P).cuda())
+    torch.cuda.synchronize()
+    got = out.cpu().numpy()
+    assert np.all(got[2] == 0.0) and (nv[1] == 1 or np.all(got[4] == 0.0))     # C_yy < 0 only matters if vy is active
+    for c in range(7):
+        assert np.max(np.abs(got[c] - ref[c])) <= TOL * max(np.max(np.abs(ref[c])), 1e-300), c
+
+
+@pytest.mark.parametrize("nx,dim", [((6, 4, 1), 0), ((4, 6, 1), 1), ((4, 4, 5), 2)])
+@pytest.mark.parametrize("side", [0, 1])
+def test_exchange_maxwellian_matches_oracle(torch_cuda, mphv, orc, nx, dim, side):
+    torch = torch_cuda
+    from paper_2305_01487_b200 import inputs
+    w = small_workload(nx, (12, 12, 8), (0, 0, 0))
+    f0, _, _, _ = inputs.make_all(w)
+    sim = mphv.Vlasov.from_workload(w)
+    grid, box = orc.Grid(w.nx, w.nv, w.bc), orc.Box(w.xlo, w.xhi, w.vlo, w.vhi)
+    plane = grid.n_space // w.nx[dim]
+    rng = np.random.default_rng(32)
+    n, j, P = _random_moments(rng, 2 * plane)
+    n_fl, j_fl, P_fl = n.reshape(2, plane), j.reshape(3, 2, plane), P.reshape(6, 2, plane)
+    ref = f0.copy()
+    orc.exchange_maxwellian(ref, grid, box, dim, side, n_fl, j_fl, P_fl)
+    f = torch.from_numpy(f0).cuda()
+    sim.bind_f(f)
+    sim.exchange_maxwellian(dim, side, torch.from_numpy(n_fl).cuda(), torch.from_numpy(j_fl).cuda(),
+                            torch.from_numpy(P_fl).cuda())
+    torch.cuda.synchronize()
+    got = f.cpu().numpy()
+    ax = {0: 2, 1: 1, 2: 0}[dim]
+    nd = w.nx[dim]
+    layers = [nd - 2, nd - 1] if side else [0, 1]
+    keep = [i for i in range(nd) if i not in layers]
+    assert np.array_equal(np.take(got, keep, axis=ax), np.take(f0, keep, axis=ax)), "interior untouched"
+    scale = np.max(np.abs(ref), axis=(3, 4, 5), keepdims=True)
+    assert np.max(np.abs(got - ref) / scale) <= TOL
+
+
+def test_maxwellian_errors(torch_cuda, mphv, orc):
+    w = small_workload((4, 4, 1), (8, 8, 8))
+    sim = mphv.Vlasov.from_workload(w)
+    with pytest.raises(mphv.MphvError) as e:
+        mphv.mphv_maxwellian(sim.ctx, 3, None, None, None, None)
+    assert e.value.code == mphv.ERR_ARG
+    with pytest.raises(mphv.MphvError) as e:
+        mphv.mphv_exchange_maxwellian(sim.ctx, 2, 0, None, None, None)      # z inactive
+    assert e.value.code == mphv.ERR_ARG
