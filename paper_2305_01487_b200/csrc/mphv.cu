@@ -298,7 +298,10 @@ int launch_vstage(mphv_ctx *c, double dt, double *n, double *j, double *P)
 }
 
 // S_x then S_y in one pass over f (mphv_sxy.cuh)
-const int SXY_NR = 6;                   // ring depth: SXY_NR - 1 rows in flight per CTA
+#ifndef MPHV_SXY_NR
+#define MPHV_SXY_NR 6
+#endif
+const int SXY_NR = MPHV_SXY_NR;         // ring depth: SXY_NR - 1 rows in flight per CTA
 
 void *sxy_fn(int C, int bcx, int bcy)
 {

@@ -32,6 +32,51 @@ __device__ __forceinline__ double march_q(double a, double b, double c, double c
     return fma(cy, lm, fma(cx, lp, b));
 }
 
+// N cell fluxes Q_m = march_q(w[m], w[m+1], w[m+2]) (STRIDE 1: sliding window) or
+// march_q(a[m], b[m], c[m]) with a WARP-UNIFORM fast path: "the limiter only for small values of the
+// phase space distribution function" -- where no lane of the warp has a slope above twice its
+// cell value (cap >= d+ and cap >= d- everywhere), lim(d) = d and Q = b + cx d+ + cy d- needs no
+// select at all (bitwise the same result: the slow path evaluates the same two fma with lp = d+, lm = d-).
+template <int N>
+__device__ __forceinline__ void march_q_window(const double *w, double cx, double cy, double *q)
+{
+    double dp[N], dm[N];
+    bool plain = true;
+#pragma unroll
+    for (int m = 0; m < N; ++m) {
+        const double b = w[m + 1], cap = b + b;
+        dp[m] = w[m + 2] - b; dm[m] = w[m] - b;
+        plain = plain && !(cap < dp[m]) && !(cap < dm[m]);
+    }
+    if (__all_sync(__activemask(), plain)) {
+#pragma unroll
+        for (int m = 0; m < N; ++m) q[m] = fma(cy, dm[m], fma(cx, dp[m], w[m + 1]));
+    } else {
+#pragma unroll
+        for (int m = 0; m < N; ++m) q[m] = march_q(w[m], w[m + 1], w[m + 2], cx, cy);
+    }
+}
+template <int N>
+__device__ __forceinline__ void march_q_lanes(const double *a, const double *b, const double *c,
+                                              double cx, double cy, double *q)
+{
+    double dp[N], dm[N];
+    bool plain = true;
+#pragma unroll
+    for (int m = 0; m < N; ++m) {
+        const double cap = b[m] + b[m];
+        dp[m] = c[m] - b[m]; dm[m] = a[m] - b[m];
+        plain = plain && !(cap < dp[m]) && !(cap < dm[m]);
+    }
+    if (__all_sync(__activemask(), plain)) {
+#pragma unroll
+        for (int m = 0; m < N; ++m) q[m] = fma(cy, dm[m], fma(cx, dp[m], b[m]));
+    } else {
+#pragma unroll
+        for (int m = 0; m < N; ++m) q[m] = march_q(a[m], b[m], c[m], cx, cy);
+    }
+}
+
 template <int VEC, int U, int KIND, int BC, bool MOM, int MINB>
 __global__ void __launch_bounds__(256, MINB)
 march2_kernel(const MarchArgs p)

@@ -126,8 +126,7 @@ sxy_kernel(const SxyArgs p)
         double w[7], q[5];
 #pragma unroll
         for (int m = 0; m < 7; ++m) w[m] = row[off[m]];
-#pragma unroll
-        for (int m = 0; m < 5; ++m) q[m] = march_q(w[m], w[m + 1], w[m + 2], xcx, xcy);
+        march_q_window<5>(w, xcx, xcy, q);
 #pragma unroll
         for (int c = 0; c < 4; ++c) nw[c] = fma(sx, q[c] - q[c + 1], posx ? w[c + 2] : w[c + 1]);
     };
@@ -156,12 +155,13 @@ sxy_kernel(const SxyArgs p)
     // one y march step: nw = g_{i+2} arrives, Q_{i+1} is formed, row i is finished and stored
     double *dst = slab + (long long)x0 * nvel + v;
     auto ystep = [&](const double (&nw)[4]) {
+        double qn[4];
+        march_q_lanes<4>(G0, G1, nw, ycx, ycy, qn);
 #pragma unroll
         for (int m = 0; m < 4; ++m) {
-            const double qn = march_q(G0[m], G1[m], nw[m], ycx, ycy);
-            const double en = Q[m] - qn;
+            const double en = Q[m] - qn[m];
             dst[m * nvel] = fma(sy, posy ? E[m] : en, G0[m]);
-            Q[m] = qn; E[m] = en;
+            Q[m] = qn[m]; E[m] = en;
             G0[m] = G1[m]; G1[m] = nw[m];
         }
         dst += row_stride;
