@@ -244,7 +244,7 @@ int vstage_ns(int variant) { return variant == CUBE_32 ? 2 : 3; }
 size_t vstage_smem_bytes(int nvx, int nvy, int nvz, int ns, int T)
 {
     const size_t cells = (size_t)nvx * nvy, xcells = (size_t)nvx * (nvy + 4);
-    return (ns * 2 * cells + VS_NXB * 2 * xcells + nvz + 320 + 8 * (size_t)T) * sizeof(double) + (ns + 2) * sizeof(uint64_t);
+    return (ns * 2 * cells + VS_NXB * 2 * xcells + nvz + 320 + 12 * (size_t)T) * sizeof(double) + (ns + 2) * sizeof(uint64_t);
 }
 
 size_t cube_smem_bytes(int nvx, int nvy, int nvz, int ns, bool reduce)

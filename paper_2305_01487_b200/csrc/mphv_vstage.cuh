@@ -46,7 +46,8 @@ vstage_kernel(const CubeArgs p)
     double *vzt = xb + (size_t)VS_NXB * 2 * xcells;                     // [nvz] vz centres
     double *red = vzt + nvz;                                            // [10][32]
     double2 *zc = reinterpret_cast<double2 *>(red + 320);               // [4][T] V_vz slope coefficients of the thread's pencils
-    uint64_t *bars = reinterpret_cast<uint64_t *>(zc + 4 * (size_t)blockDim.x);   // [NS] TMA full, [2] xbar
+    double *zsm = reinterpret_cast<double *>(zc + 4 * (size_t)blockDim.x);         // [4][T] V_vz Courant numbers of the thread's pencils
+    uint64_t *bars = reinterpret_cast<uint64_t *>(zsm + 4 * (size_t)blockDim.x);   // [NS] TMA full, [2] xbar
 
     const long long c_begin = (p.ns * (long long)blockIdx.x) / gridDim.x;
     const long long c_end = (p.ns * ((long long)blockIdx.x + 1)) / gridDim.x;
@@ -90,12 +91,13 @@ vstage_kernel(const CubeArgs p)
     // per-cube linear forms of the Courant numbers: s = a + vz b
     double ax = 0.0, bx = 0.0, ay = 0.0, by = 0.0;
     // V_vz march state of this thread's 4 pencils (rows r0..r0+3 of column jx)
-    double zs[4];                                    // s; the coefficients of lim(g_{j+1}-g_j), lim(g_{j-1}-g_j) live in zc
+    // s and the coefficients of lim(g_{j+1}-g_j), lim(g_{j-1}-g_j) live in zsm, zc
     double2 *const zcp = zc + tid;                   // (shared memory, written and read by this thread only)
+    double *const zsp = zsm + tid;
     double G0[4], G1[4], Q[4], E[4];                 // g_i, g_{i+1}, Q_i, E_i = Q_{i-1} - Q_i
     double P0 = 0.0, Q1 = 0.0, Q2 = 0.0, Z1 = 0.0, Z2 = 0.0, ZQ = 0.0;   // moment sums (see header)
 #pragma unroll
-    for (int m = 0; m < 4; ++m) { zs[m] = 0.0; G0[m] = G1[m] = Q[m] = E[m] = 0.0; }
+    for (int m = 0; m < 4; ++m) { G0[m] = G1[m] = Q[m] = E[m] = 0.0; }
 
     // One march step for the 4 pencils: nw = g_{i+2} arrives, Q_{i+1} is formed, cell i is finished
     // and stored to plane i (po). MODE 0: interior; 1: i = nvz-2 (Q_{i+1} sits in front of the high
@@ -105,13 +107,14 @@ vstage_kernel(const CubeArgs p)
         double o[4];
 #pragma unroll
         for (int m = 0; m < 4; ++m) {
-            const bool pos = __double2hiint(zs[m]) >= 0;
+            const double zs = zsp[m * blockDim.x];
+            const bool pos = __double2hiint(zs) >= 0;
             const double2 zxy = zcp[m * blockDim.x];
             double qn = march_q(G0[m], G1[m], nw[m], zxy.x, zxy.y);
             if (MODE == 1 && pos) qn = 0.0;
             if (MODE == 2 && !pos) qn = 0.0;
             const double en = Q[m] - qn;
-            o[m] = fma(zs[m], pos ? E[m] : en, G0[m]);
+            o[m] = fma(zs, pos ? E[m] : en, G0[m]);
             Q[m] = qn; E[m] = en;
             G0[m] = G1[m]; G1[m] = nw[m];
             po[m * nvx] = o[m];
@@ -195,7 +198,7 @@ vstage_kernel(const CubeArgs p)
                 double c1, nc2;
                 courant_poly(s, c1, nc2);
                 const bool pos = __double2hiint(s) >= 0;
-                zs[m] = s;
+                zsp[m * blockDim.x] = s;
                 zcp[m * blockDim.x] = pos ? make_double2(c1, nc2) : make_double2(nc2, c1);
             }
             P0 = Q1 = Q2 = Z1 = Z2 = ZQ = 0.0;
@@ -229,7 +232,7 @@ vstage_kernel(const CubeArgs p)
                     } else {
 #pragma unroll
                         for (int m = 0; m < 4; ++m) {                    // g_1: Q_0, E_0 (face -1/2 carries no flux)
-                            const bool pos = __double2hiint(zs[m]) >= 0;
+                            const bool pos = __double2hiint(zsp[m * blockDim.x]) >= 0;
                             G1[m] = nw[m];
                             const double2 zxy = zcp[m * blockDim.x];
                             double q0 = march_q(0.0, G0[m], G1[m], zxy.x, zxy.y);
