@@ -10,7 +10,8 @@ N = 1 runs BASELINE.json configs[3] (2D3V 128x64x40^3, the headline roofline con
 N > 1 (torchrun): weak scaling by spatial block decomposition (the paper's own
 parallelisation): the periodic x axis is N times longer, every rank owns one
 configs[3]-sized block and exchanges its two boundary layers with both x neighbours before the
-S_x sweep (mphv_pack_halo -> NCCL send/recv -> mphv_sweep_x_halo); time = max over ranks.
+X stage (mphv_pack_halo -> NCCL send/recv -> mphv_stage_x_halo: S_x with the received ghost layers and S_y
+in one pass); time = max over ranks.
 --decomp none instead runs N independent seeded problems (no exchange); --decomp halo at N = 1
 sends the spatial sweeps through the same pack / halo kernels with the block as its own neighbour.
 --impl reference times the CPU oracle (oracle/) on a bounded spatial sub-block of the same
@@ -228,7 +229,7 @@ def run_mphv(args, w):
     peak_gbs, peak_src = (float(peaks["hbm_gbs"]), "measured") if "hbm_gbs" in peaks else (6650.0, "fallback")
 
     if halo_mode:
-        dv = halo.DistributedVlasov(wg, dec, rank, dev, force_halo=(world == 1))
+        dv = halo.DistributedVlasov(wg, dec, rank, dev, force_halo=(0,) if world == 1 else False)
         sim = dv.sim
         step_moments = dv.step_moments
     else:

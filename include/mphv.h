@@ -114,6 +114,12 @@ int mphv_step(mphv_ctx *ctx, double dt);
  * mphv_stage_v this gives callers true Strang splitting, X(dt/2) V(dt) X(dt/2). */
 int mphv_stage_x(mphv_ctx *ctx, double dt);
 
+/* The X stage of a block that is decomposed along x ONLY (the other spatial axes are whole and follow
+ * grid.bc): S_x with its ghost cells from lo_dev / hi_dev (as mphv_sweep_x_halo(0, ...); NULL = global
+ * outflow end), then S_y, S_z; S_x and S_y fused into one pass as in mphv_step where the grid allows.
+ * Same checks as mphv_sweep_x_halo for axis 0 and mphv_sweep_x for the others. */
+int mphv_stage_x_halo(mphv_ctx *ctx, double dt, const double *lo_dev, const double *hi_dev);
+
 /* The V stage of mphv_step alone: V_vx, V_vy, V_vz in that order (fused as in mphv_step), and, when
  * n_dev is not NULL, the moments of the result (then j_dev and P_dev must be given too). With
  * mphv_sweep_x / mphv_sweep_x_halo for the X stage this is mphv_step[_moments] taken apart, for callers

@@ -303,24 +303,25 @@ int launch_vstage(mphv_ctx *c, double dt, double *n, double *j, double *P)
 #endif
 const int SXY_NR = MPHV_SXY_NR;         // ring depth: SXY_NR - 1 rows in flight per CTA
 
+enum { SXY_BCX_HALO = 2 };             // bcx argument of sxy_fn beyond MPHV_BC_PERIODIC / MPHV_BC_OUTFLOW
 void *sxy_fn(int C, int bcx, int bcy)
 {
+#define SXY_ROW(CC, TM, MB, BX) \
+    (bcy == MPHV_BC_PERIODIC ? (void *)sxy_kernel<CC, SXY_NR, BX, BC_PER, TM, MB> : (void *)sxy_kernel<CC, SXY_NR, BX, BC_OUT, TM, MB>)
 #define SXY_PICK(CC, TM, MB) \
-    (bcx == MPHV_BC_PERIODIC ? (bcy == MPHV_BC_PERIODIC ? (void *)sxy_kernel<CC, SXY_NR, BC_PER, BC_PER, TM, MB> \
-                                                         : (void *)sxy_kernel<CC, SXY_NR, BC_PER, BC_OUT, TM, MB>) \
-                             : (bcy == MPHV_BC_PERIODIC ? (void *)sxy_kernel<CC, SXY_NR, BC_OUT, BC_PER, TM, MB> \
-                                                         : (void *)sxy_kernel<CC, SXY_NR, BC_OUT, BC_OUT, TM, MB>))
+    (bcx == MPHV_BC_PERIODIC ? SXY_ROW(CC, TM, MB, BC_PER) : bcx == MPHV_BC_OUTFLOW ? SXY_ROW(CC, TM, MB, BC_OUT) : SXY_ROW(CC, TM, MB, BC_HALO))
     return C == 16 ? SXY_PICK(16, 512, 1) : SXY_PICK(8, 256, 2);
 #undef SXY_PICK
+#undef SXY_ROW
 }
 
-size_t sxy_smem_bytes(int C, int nx, int T, bool per_y)
+size_t sxy_smem_bytes(int C, int nx, int T, bool per_y)             // sized for the halo variant (nx + 4 cells per row)
 {
-    const size_t rowd = C == 16 ? sxy_row_doubles<16>(nx) : sxy_row_doubles<8>(nx);
+    const size_t rowd = C == 16 ? sxy_row_doubles<16>(nx + 4) : sxy_row_doubles<8>(nx + 4);
     return (SXY_NR * rowd + (per_y ? 8 * (size_t)T : 0)) * sizeof(double);
 }
 
-int launch_sxy(mphv_ctx *c, double dt)
+int launch_sxy(mphv_ctx *c, double dt, bool halo = false, const double *lo = nullptr, const double *hi = nullptr)
 {
     SxyArgs a;
     std::memset(&a, 0, sizeof a);
@@ -331,7 +332,8 @@ int launch_sxy(mphv_ctx *c, double dt)
     a.dt = dt; a.dx = c->dx[0]; a.dy = c->dx[1];
     a.g = c->gd;
     Timed tm(c, SLOT_SXY, 32.0 * (double)c->nf);
-    void *fn = sxy_fn(c->sxy_C, c->grid.bc[0], c->grid.bc[1]);
+    a.halo_lo = lo; a.halo_hi = hi;
+    void *fn = sxy_fn(c->sxy_C, halo ? SXY_BCX_HALO : c->grid.bc[0], c->grid.bc[1]);
     void *args[] = { &a };
     const unsigned grid = (unsigned)((long long)c->grid.nx[2] * a.chunks);
     cudaError_t e = cudaLaunchKernel(fn, dim3(grid), dim3((unsigned)c->sxy_T), args, c->sxy_smem, c->stream);
@@ -691,7 +693,7 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
             for (int by = 0; by < 2 && ok; ++by) {
                 const size_t sm = sxy_smem_bytes(C, nx, T, by == MPHV_BC_PERIODIC);
                 if (by == grid->bc[1]) smem = sm;
-                for (int bx = 0; bx < 2 && ok; ++bx)
+                for (int bx = 0; bx < 3 && ok; ++bx)
                     ok = sm <= (size_t)max_optin &&
                          cudaFuncSetAttribute(sxy_fn(C, bx, by), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) == cudaSuccess;
             }
@@ -908,6 +910,35 @@ int mphv_exchange_maxwellian(mphv_ctx *c, int dim, int side, const double *n_fl,
     Timed tm(c, SLOT_EXCH, 2.0 * (double)a.plane * 16.0 * (double)c->nvel);
     exchange_kernel<<<(unsigned)(2 * a.plane), block, 0, c->stream>>>(a);
     return after_launch(c, "exchange_kernel");
+}
+
+int mphv_stage_x_halo(mphv_ctx *c, double dt, const double *lo, const double *hi)
+{
+    int st = check_common(c, dt, false);
+    if (st != MPHV_OK) return st;
+    if (c->grid.nx[0] < 2) { set_err(c, "spatial dim 0 is inactive"); return MPHV_ERR_ARG; }
+    if (((uintptr_t)lo & 15) || ((uintptr_t)hi & 15)) { set_err(c, "halo buffers must be 16-byte aligned"); return MPHV_ERR_ARG; }
+    if (c->grid.bc[0] == MPHV_BC_PERIODIC && (!lo || !hi)) {
+        set_err(c, "stage_x_halo: a periodic x axis needs both halo buffers"); return MPHV_ERR_ARG;
+    }
+    if (!(max_courant_x(c, 0, dt) < 1.0)) {
+        set_err(c, "spatial sweep 0 with halos: max |s| = %g >= 1 reaches past the two boundary cells", max_courant_x(c, 0, dt));
+        return MPHV_ERR_RANGE;
+    }
+    for (int d = 1; d < 3; ++d)
+        if (c->grid.nx[d] > 1 && (st = range_x(c, d, dt)) != MPHV_OK) return st;
+    int d0 = 1;
+    if (c->fusion >= 3 && c->sxy_T > 0 && c->grid.nx[1] > 1 && max_courant_x(c, 1, dt) < 1.0) {
+        if ((st = launch_sxy(c, dt, true, lo, hi)) != MPHV_OK) return st;          // S_x (ghosts from the slabs), S_y
+        d0 = 2;
+    } else {
+        MarchArgs a = march_args_space(c, 0, dt);
+        a.halo_lo = lo; a.halo_hi = hi;
+        if ((st = launch_march<KIND_SPACE, BC_HALO>(c, a)) != MPHV_OK) return st;
+    }
+    for (int d = d0; d < 3; ++d)
+        if (c->grid.nx[d] > 1 && (st = do_sweep_x(c, d, dt)) != MPHV_OK) return st;
+    return MPHV_OK;
 }
 
 int mphv_step_moments(mphv_ctx *c, double dt, double *n, double *j, double *P)

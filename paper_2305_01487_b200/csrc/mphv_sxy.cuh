@@ -19,7 +19,9 @@
 // Periodic y: the rows ny-2, ny-1 are produced first (and again at the end of the stream, before
 // they are overwritten), the S_x images of rows 0, 1 are kept for the wrap. Outflow: zero-gradient
 // ghosts (R6). Boundary handling in x is index math on the 7 shared-memory offsets of a thread.
-// Requires nx % 4 == 0, nvel % C == 0, |s| < 1 on both axes; other cases use the march kernels.
+// BCX = BC_HALO: the block is one of several along x; the ghost cells of every row come from the
+// neighbours' packed boundary layers. Requires nx % 4 == 0, nvel % C == 0, |s| < 1 on both axes; other
+// cases use the march kernels.
 #pragma once
 #include "mphv_vstage.cuh"
 
@@ -31,6 +33,9 @@ struct SxyArgs {
     int chunks;             // nvel / C
     long long nvel;         // doubles between x neighbours
     double dt, dx, dy;
+    // BCX == BC_HALO (block decomposition along x): the two ghost layers below / above the block,
+    // each [nz ny][2][nvel] as packed by pack_halo_kernel; NULL = global outflow end (zero-gradient ghosts, R6)
+    const double *halo_lo, *halo_hi;
     GridDev g;
 };
 
@@ -62,7 +67,8 @@ sxy_kernel(const SxyArgs p)
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double *ring = reinterpret_cast<double *>(smem_raw);                 // [NR][rowd]
     const int nx = p.nx, ny = p.ny;
-    const int rowd = sxy_row_doubles<C>(nx);
+    constexpr int XS = BCX == BC_HALO ? 2 : 0;                           // ring rows carry 2 + 2 ghost cells
+    const int rowd = sxy_row_doubles<C>(nx + 2 * XS);
     const int tid = threadIdx.x, T = blockDim.x;                         // T = (nx / 4) * C
     double *keep = ring + (size_t)NR * rowd;                             // [2][4][T] (periodic y only)
     const int v = tid % C, xq = tid / C;
@@ -93,8 +99,12 @@ sxy_kernel(const SxyArgs p)
     for (int m = 0; m < 7; ++m) {
         int xi = x0 - 2 + (posx ? 0 : 1) + m;
         if (BCX == BC_PER) { if (xi < 0) xi += nx; else if (xi >= nx) xi -= nx; }
-        else               { xi = xi < 0 ? 0 : (xi >= nx ? nx - 1 : xi); }
-        off[m] = sxy_xoff<C>(xi) + v;
+        else if (BCX == BC_OUT) { xi = xi < 0 ? 0 : (xi >= nx ? nx - 1 : xi); }
+        else {
+            if (xi < 0 && !p.halo_lo) xi = 0;
+            if (xi >= nx && !p.halo_hi) xi = nx - 1;
+        }
+        off[m] = sxy_xoff<C>(xi + XS) + v;
     }
 
     // ---- row stream: production k brings row row_of(k); K productions
@@ -107,7 +117,14 @@ sxy_kernel(const SxyArgs p)
         for (int u = 0; u < 2; ++u) {                                    // nx C / 2 pieces of 16 bytes = 2 T
             const int piece = tid + u * T;
             const int x = piece / (C / 2), part = piece % (C / 2);
-            cp_async16(dst + sxy_xoff<C>(x) + 2 * part, src + (long long)x * nvel + 2 * part);
+            cp_async16(dst + sxy_xoff<C>(x + XS) + 2 * part, src + (long long)x * nvel + 2 * part);
+        }
+        if (BCX == BC_HALO && tid < 4 * (C / 2)) {                       // the 2 + 2 ghost cells of the row
+            const int hx = tid / (C / 2), part = tid % (C / 2);
+            const double *h = hx < 2 ? p.halo_lo : p.halo_hi;
+            if (h)
+                cp_async16(dst + sxy_xoff<C>(hx < 2 ? hx : nx + hx) + 2 * part,
+                           h + ((o * ny + row_of(k)) * 2 + (hx & 1)) * nvel + (long long)chunk * C + 2 * part);
         }
     };
 #pragma unroll

@@ -154,9 +154,10 @@ class DistributedVlasov:
     buffers and the exchange. step / step_moments give, block by block, the result of the single-GPU
     mphv_step on the whole grid (same kernels; ghost cells from the neighbours)."""
 
-    def __init__(self, w_global, decomp: Decomp, rank: int, device, group=None, force_halo: bool = False):
-        """force_halo: route EVERY active spatial sweep through pack -> exchange -> halo kernel, also along
-        axes a single rank owns (periodic: the block is its own neighbour; outflow: no neighbour)."""
+    def __init__(self, w_global, decomp: Decomp, rank: int, device, group=None, force_halo=False):
+        """force_halo: True routes EVERY active spatial sweep through pack -> exchange -> halo kernel, also
+        along axes a single rank owns (periodic: the block is its own neighbour; outflow: no neighbour);
+        a tuple of axes does so for those axes only."""
         import torch
         from . import mphv
         self.torch = torch
@@ -165,7 +166,8 @@ class DistributedVlasov:
         self.sim = mphv.Vlasov.from_workload(self.w, device=device)
         self.xchg = HaloExchange(decomp, rank, group)
         self.buf = {}
-        self.use_halo = [self.w.nx[d] > 1 and (force_halo or decomp.needs_exchange(d)) for d in range(3)]
+        forced = (0, 1, 2) if force_halo is True else tuple(force_halo or ())
+        self.use_halo = [self.w.nx[d] > 1 and (d in forced or decomp.needs_exchange(d)) for d in range(3)]
         for d in range(3):
             if self.use_halo[d]:
                 cnt = self.sim.halo_count(d)
@@ -191,9 +193,17 @@ class DistributedVlasov:
         self.step_moments(dt, None)
 
     def step_moments(self, dt: float, out=None):
-        for d in range(3):
-            if self.w.nx[d] > 1:
-                self.sweep_x(d, dt)
+        if self.use_halo[0] and not self.use_halo[1] and not self.use_halo[2]:
+            # decomposed along x only: one exchange, then the whole X stage (S_x and S_y in one pass)
+            send_lo, send_hi, recv_lo, recv_hi = self.buf[0]
+            self.sim.pack_halo(0, 0, send_lo)
+            self.sim.pack_halo(0, 1, send_hi)
+            has_lo, has_hi = self.xchg.exchange(0, send_lo, send_hi, recv_lo, recv_hi)
+            self.sim.stage_x_halo(dt, recv_lo if has_lo else None, recv_hi if has_hi else None)
+        else:
+            for d in range(3):
+                if self.w.nx[d] > 1:
+                    self.sweep_x(d, dt)
         return self.sim.stage_v(dt, out)
 
     def alloc_moments(self):

@@ -27,7 +27,7 @@ SYMBOLS = (
     "mphv_moments", "mphv_step_moments", "mphv_run_host", "mphv_sum_f", "mphv_launch_count",
     "mphv_set_fusion", "mphv_set_vmode", "mphv_maxwellian", "mphv_exchange_maxwellian", "mphv_strerror", "mphv_last_error",
     "mphv_set_timing", "mphv_timing_slots", "mphv_get_timing",
-    "mphv_stage_x", "mphv_stage_v", "mphv_halo_count", "mphv_pack_halo", "mphv_sweep_x_halo",
+    "mphv_stage_x", "mphv_stage_x_halo", "mphv_stage_v", "mphv_halo_count", "mphv_pack_halo", "mphv_sweep_x_halo",
 )
 
 
@@ -83,6 +83,7 @@ def lib() -> C.CDLL:
         "mphv_get_timing": (i32, [vp, i32, C.c_char_p, C.c_size_t, C.POINTER(dbl),
                                   C.POINTER(C.c_uint64), C.POINTER(dbl)]),
         "mphv_stage_x": (i32, [vp, dbl]),
+        "mphv_stage_x_halo": (i32, [vp, dbl, vp, vp]),
         "mphv_stage_v": (i32, [vp, dbl, vp, vp, vp]),
         "mphv_halo_count": (C.c_size_t, [vp, i32]),
         "mphv_pack_halo": (i32, [vp, i32, i32, vp]),
@@ -174,6 +175,10 @@ def mphv_step_moments(ctx, dt: float, n_dev: int, j_dev: int, P_dev: int):
 
 def mphv_stage_x(ctx, dt: float):
     _check(ctx, lib().mphv_stage_x(ctx, float(dt)))
+
+
+def mphv_stage_x_halo(ctx, dt: float, lo_dev, hi_dev):
+    _check(ctx, lib().mphv_stage_x_halo(ctx, float(dt), lo_dev, hi_dev))
 
 
 def mphv_stage_v(ctx, dt: float, n_dev=None, j_dev=None, P_dev=None):
@@ -320,6 +325,9 @@ class Vlasov:
 
     def stage_x(self, dt):
         mphv_stage_x(self.ctx, dt)
+
+    def stage_x_halo(self, dt, lo=None, hi=None):
+        mphv_stage_x_halo(self.ctx, dt, None if lo is None else lo.data_ptr(), None if hi is None else hi.data_ptr())
 
     def stage_v(self, dt, out=None):
         """The V stage alone; with out = (n, j, P) tensors the moments of the result are written too."""
