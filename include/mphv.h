@@ -202,6 +202,14 @@ int mphv_maxwellian(mphv_ctx *ctx, size_t count, const double *n_dev, const doub
 int mphv_exchange_maxwellian(mphv_ctx *ctx, int dim, int side, const double *n_fl_dev,
                              const double *j_fl_dev, const double *P_fl_dev);
 
+/* Matching the ten moments of the bound f to given ones by exchanging Maxwellians, in every spatial
+ * cell, in place ("matched-moments Vlasov solver", "exchanging Maxwellians"; reading R18):
+ *     f <- M[n_t, j_t, P_t] + (f - M[moments of f]).
+ * n_t_dev [ns], j_t_dev [3][ns], P_t_dev [6][ns] in the layouts of mphv_moments. The time-step order of the
+ * paper's Algorithm 1 and its density correction are missing from PAPER.md and not reproduced;
+ * positivity of the result is the caller's concern. Only enqueues. */
+int mphv_match_moments(mphv_ctx *ctx, const double *n_t_dev, const double *j_t_dev, const double *P_t_dev);
+
 /* Mode of the V stage. MPHV_V_PLAIN (default; BASELINE.json north_star): three plain 1-D sweeps with
  * the Courant numbers a_d dt / dv_d, a = (q/m)(E + v x B) at the cell centres. MPHV_V_BACKSUB: "The
  * velocity space splitting is realized via backsubstitution" (sec. 4.1; reading R15 of

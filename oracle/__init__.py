@@ -7,6 +7,6 @@ Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline``
 from .binding import (  # noqa: F401
     Grid, Box, build, lib, sweep_pencil, sweep_x, sweep_v, step, moments, total, num_threads,
     boris_map, backsub_foot, sweep_pencil_faces, sweep_v_backsub, step_backsub,
-    maxwellian, exchange_maxwellian,
+    maxwellian, exchange_maxwellian, match_moments,
     BC_PERIODIC, BC_OUTFLOW, BC_WALL, OK, ERR_ARG, ERR_RANGE,
 )

@@ -116,6 +116,8 @@ def lib() -> C.CDLL:
         L.orc_maxwellian.restype = C.c_int
         L.orc_exchange_maxwellian.argtypes = [dp, C.POINTER(_CGrid), C.POINTER(_CBox), C.c_int, C.c_int, dp, dp, dp]
         L.orc_exchange_maxwellian.restype = C.c_int
+        L.orc_match_moments.argtypes = [dp, C.POINTER(_CGrid), C.POINTER(_CBox), dp, dp, dp]
+        L.orc_match_moments.restype = C.c_int
         L.orc_num_threads.argtypes = []
         L.orc_num_threads.restype = C.c_int
         _lib = L
@@ -265,6 +267,18 @@ def exchange_maxwellian(f: np.ndarray, grid: Grid, box: Box, dim: int, side: int
     st = lib().orc_exchange_maxwellian(_p(f), C.byref(g), C.byref(b), int(dim), int(side), _p(n_fl), _p(j_fl), _p(P_fl))
     if st != OK:
         raise ValueError(f"orc_exchange_maxwellian status {st}")
+
+
+def match_moments(f: np.ndarray, grid: Grid, box: Box, n_t, j_t, P_t) -> None:
+    """f <- M[n_t, j_t, P_t] + (f - M[moments of f]) in every spatial cell, in place."""
+    _check_f(f, grid)
+    n_t = np.ascontiguousarray(n_t, dtype=np.float64); assert n_t.size == grid.n_space
+    j_t = np.ascontiguousarray(j_t, dtype=np.float64); assert j_t.size == 3 * grid.n_space
+    P_t = np.ascontiguousarray(P_t, dtype=np.float64); assert P_t.size == 6 * grid.n_space
+    g, b = grid.c(), box.c()
+    st = lib().orc_match_moments(_p(f), C.byref(g), C.byref(b), _p(n_t), _p(j_t), _p(P_t))
+    if st != OK:
+        raise ValueError(f"orc_match_moments status {st}")
 
 
 def total(f: np.ndarray) -> float:

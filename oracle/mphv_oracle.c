@@ -770,6 +770,40 @@ int orc_exchange_maxwellian(double *f, const orc_grid *g, const orc_box *b, int 
     return ORC_OK;
 }
 
+/*
+ * Matching the ten moments of f to given ones by exchanging Maxwellians, in every spatial cell
+ * (in part). P:L137: "the matched-moments Vlasov solver [33] is utilized";
+ * "the way of adjusting the distribution function is now done by exchanging Maxwellians [33].
+ * We remove the ten-moment Maxwellian part from the ... Vlasov data and add the result ... to the
+ * Maxwellian computed from the fluid ... data." Reading R18: per cell
+ *     f  <-  M[n_t, j_t, P_t] + (f - M[moments of f]),
+ * the exchange of P:L187 with sigma = 1 applied to the cell itself. Algorithm 1 (the order of these
+ * calls inside the matched-moments time step, and the density correction of P:L163) is missing from
+ * PAPER.md and is NOT reproduced. n_t [ns], j_t [3][ns], P_t [6][ns] in the layouts of orc_moments.
+ */
+int orc_match_moments(double *f, const orc_grid *g, const orc_box *b,
+                      const double *n_t, const double *j_t, const double *P_t)
+{
+    if (!f || !grid_ok(g, b) || !n_t || !j_t || !P_t) return ORC_ERR_ARG;
+    const size_t ns = n_space(g), nvel = n_vel(g);
+    double *Mt = (double *)malloc(nvel * sizeof(double));
+    double *Mf = (double *)malloc(nvel * sizeof(double));
+    if (!Mt || !Mf) { free(Mt); free(Mf); return ORC_ERR_ARG; }
+    for (size_t c = 0; c < ns; ++c) {
+        double *cube = f + c * nvel;
+        double nf, jf[3], Pf[6];
+        cube_moments(g, b, cube, &nf, jf, Pf);
+        maxwellian_cube(g, b, nf, jf, Pf, Mf);
+        double jt[3] = { j_t[c], j_t[ns + c], j_t[2 * ns + c] };
+        double Pt[6];
+        for (int a = 0; a < 6; ++a) Pt[a] = P_t[(size_t)a * ns + c];
+        maxwellian_cube(g, b, n_t[c], jt, Pt, Mt);
+        for (size_t e = 0; e < nvel; ++e) cube[e] = Mt[e] + (cube[e] - Mf[e]);
+    }
+    free(Mt); free(Mf);
+    return ORC_OK;
+}
+
 /* Sum of all entries of f in long double (mass in units of cell volume). */
 double orc_sum(const double *f, size_t count)
 {

@@ -52,11 +52,11 @@ struct mphv_ctx {
 };
 
 enum { SLOT_SX0 = 0, SLOT_SX1, SLOT_SX2, SLOT_VX, SLOT_VY, SLOT_VZ, SLOT_MOM, SLOT_VXY, SLOT_VZMOM,
-       SLOT_SHIFT, SLOT_SUM, SLOT_AMAX, SLOT_VCUBE, SLOT_VCUBE_MOM, SLOT_PACK, SLOT_SXY, SLOT_BSCOEF, SLOT_MAXW, SLOT_EXCH, SLOT_COUNT };
+       SLOT_SHIFT, SLOT_SUM, SLOT_AMAX, SLOT_VCUBE, SLOT_VCUBE_MOM, SLOT_PACK, SLOT_SXY, SLOT_BSCOEF, SLOT_MAXW, SLOT_EXCH, SLOT_MATCH, SLOT_COUNT };
 static const char *const SLOT_NAMES[SLOT_COUNT] = {
     "sweep_x0", "sweep_x1", "sweep_x2", "sweep_vx", "sweep_vy", "sweep_vz", "moments",
     "fused_vx_vy", "fused_vz_moments", "shift_periodic", "sum_f", "amax_fields",
-    "fused_vx_vy_vz", "fused_vx_vy_vz_moments", "pack_halo", "fused_sx_sy", "backsub_coefficients", "maxwellian", "exchange_maxwellian" };
+    "fused_vx_vy_vz", "fused_vx_vy_vz_moments", "pack_halo", "fused_sx_sy", "backsub_coefficients", "maxwellian", "exchange_maxwellian", "match_moments" };
 
 namespace {
 
@@ -910,6 +910,21 @@ int mphv_exchange_maxwellian(mphv_ctx *c, int dim, int side, const double *n_fl,
     Timed tm(c, SLOT_EXCH, 2.0 * (double)a.plane * 16.0 * (double)c->nvel);
     exchange_kernel<<<(unsigned)(2 * a.plane), block, 0, c->stream>>>(a);
     return after_launch(c, "exchange_kernel");
+}
+
+int mphv_match_moments(mphv_ctx *c, const double *n_t, const double *j_t, const double *P_t)
+{
+    if (!c) return MPHV_ERR_ARG;
+    if (!n_t || !j_t || !P_t) { set_err(c, "n_t_dev, j_t_dev or P_t_dev is NULL"); return MPHV_ERR_ARG; }
+    if (!c->f) { set_err(c, "f not bound (mphv_bind_f)"); return MPHV_ERR_STATE; }
+    MatchArgs a;
+    a.f = c->f; a.n_t = n_t; a.j_t = j_t; a.P_t = P_t; a.g = c->gd;
+    const long long plane_v = (long long)c->grid.nv[0] * c->grid.nv[1];
+    int block = 512;
+    while (block > 32 && block / 2 >= plane_v) block /= 2;
+    Timed tm(c, SLOT_MATCH, 24.0 * (double)c->nf);
+    match_kernel<<<(unsigned)c->ns, block, 0, c->stream>>>(a);
+    return after_launch(c, "match_kernel");
 }
 
 int mphv_stage_x_halo(mphv_ctx *c, double dt, const double *lo, const double *hi)

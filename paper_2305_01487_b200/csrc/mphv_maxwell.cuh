@@ -154,4 +154,65 @@ exchange_kernel(const ExchArgs p)
     }
 }
 
+// ---------------------------------------------------------------- moment matching (R18)
+// f <- M[n_t, j_t, P_t] + (f - M[moments of f]) in every spatial cell, in place: one CTA per cell, the
+// cube is read twice (moments, then the update; the second read comes from L2 for the cubes still resident).
+struct MatchArgs {
+    double *f;
+    const double *n_t, *j_t, *P_t;      // [ns], [3][ns], [6][ns]
+    GridDev g;
+};
+
+__global__ void __launch_bounds__(512)
+match_kernel(const MatchArgs p)
+{
+    __shared__ double red[10 * 32];
+    __shared__ MaxwCoef sm[2];
+    const GridDev &g = p.g;
+    const long long cell = blockIdx.x, ns = g.ns;
+    double *cube = p.f + cell * g.nvel;
+    const int plane = g.nv[0] * g.nv[1];
+    double m[10];
+#pragma unroll
+    for (int k = 0; k < 10; ++k) m[k] = 0.0;
+    for (int pos = threadIdx.x; pos < plane; pos += blockDim.x) {
+        const int jy = pos / g.nv[0], jx = pos - jy * g.nv[0];
+        const double vx = vcentre(g, 0, jx), vy = vcentre(g, 1, jy);
+        double s0 = 0.0, s1 = 0.0, s2 = 0.0;
+        for (int jz = 0; jz < g.nv[2]; ++jz) {
+            const double fv = cube[(long long)jz * plane + pos];
+            const double vz = vcentre(g, 2, jz);
+            const double t = vz * fv;
+            s0 += fv; s1 += t; s2 = fma(vz, t, s2);
+        }
+        const double x0 = vx * s0, y0 = vy * s0;
+        m[0] += s0;
+        m[1] += x0; m[2] += y0; m[3] += s1;
+        m[4] = fma(vx, x0, m[4]); m[5] = fma(vx, y0, m[5]); m[6] = fma(vx, s1, m[6]);
+        m[7] = fma(vy, y0, m[7]); m[8] = fma(vy, s1, m[8]); m[9] += s2;
+    }
+    block_reduce_sum<10>(m, red);
+    if (threadIdx.x == 0) {
+        const double dV = g.dv[0] * g.dv[1] * g.dv[2];
+        sm[0] = maxw_setup(g, m[0] * dV, m[1] * dV, m[2] * dV, m[3] * dV, m[4] * dV, m[5] * dV, m[6] * dV,
+                           m[7] * dV, m[8] * dV, m[9] * dV);
+        sm[1] = maxw_setup(g, p.n_t[cell], p.j_t[cell], p.j_t[ns + cell], p.j_t[2 * ns + cell],
+                           p.P_t[cell], p.P_t[ns + cell], p.P_t[2 * ns + cell], p.P_t[3 * ns + cell],
+                           p.P_t[4 * ns + cell], p.P_t[5 * ns + cell]);
+    }
+    __syncthreads();
+    const MaxwCoef mf = sm[0], mt = sm[1];
+    for (int pos = threadIdx.x; pos < plane; pos += blockDim.x) {
+        const int jy = pos / g.nv[0], jx = pos - jy * g.nv[0];
+        const double vx = vcentre(g, 0, jx), vy = vcentre(g, 1, jy);
+        for (int jz = 0; jz < g.nv[2]; ++jz) {
+            const double vz = vcentre(g, 2, jz);
+            const double a = mt.norm > 0.0 ? maxw_eval(mt, vx, vy, vz) : 0.0;
+            const double b = mf.norm > 0.0 ? maxw_eval(mf, vx, vy, vz) : 0.0;
+            double *q = cube + (long long)jz * plane + pos;
+            *q = a + (*q - b);
+        }
+    }
+}
+
 }  // namespace mphv

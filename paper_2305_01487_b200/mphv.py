@@ -25,7 +25,7 @@ SYMBOLS = (
     "mphv_create", "mphv_destroy", "mphv_set_stream", "mphv_f_count", "mphv_space_count",
     "mphv_bind_f", "mphv_set_fields", "mphv_sweep_x", "mphv_sweep_v", "mphv_step",
     "mphv_moments", "mphv_step_moments", "mphv_run_host", "mphv_sum_f", "mphv_launch_count",
-    "mphv_set_fusion", "mphv_set_vmode", "mphv_maxwellian", "mphv_exchange_maxwellian", "mphv_strerror", "mphv_last_error",
+    "mphv_set_fusion", "mphv_set_vmode", "mphv_maxwellian", "mphv_exchange_maxwellian", "mphv_match_moments", "mphv_strerror", "mphv_last_error",
     "mphv_set_timing", "mphv_timing_slots", "mphv_get_timing",
     "mphv_stage_x", "mphv_stage_x_halo", "mphv_stage_v", "mphv_halo_count", "mphv_pack_halo", "mphv_sweep_x_halo",
 )
@@ -78,6 +78,7 @@ def lib() -> C.CDLL:
         "mphv_set_vmode": (i32, [vp, i32]),
         "mphv_maxwellian": (i32, [vp, C.c_size_t, vp, vp, vp, vp]),
         "mphv_exchange_maxwellian": (i32, [vp, i32, i32, vp, vp, vp]),
+        "mphv_match_moments": (i32, [vp, vp, vp, vp]),
         "mphv_set_timing": (i32, [vp, i32]),
         "mphv_timing_slots": (i32, []),
         "mphv_get_timing": (i32, [vp, i32, C.c_char_p, C.c_size_t, C.POINTER(dbl),
@@ -214,6 +215,10 @@ V_PLAIN, V_BACKSUB = 0, 1
 
 def mphv_maxwellian(ctx, count: int, n_dev, j_dev, P_dev, f_out_dev):
     _check(ctx, lib().mphv_maxwellian(ctx, int(count), n_dev, j_dev, P_dev, f_out_dev))
+
+
+def mphv_match_moments(ctx, n_t_dev, j_t_dev, P_t_dev):
+    _check(ctx, lib().mphv_match_moments(ctx, n_t_dev, j_t_dev, P_t_dev))
 
 
 def mphv_exchange_maxwellian(ctx, dim: int, side: int, n_fl_dev, j_fl_dev, P_fl_dev):
@@ -374,6 +379,9 @@ class Vlasov:
             out = torch.empty((count, self.nv[2], self.nv[1], self.nv[0]), dtype=torch.float64, device=n.device)
         mphv_maxwellian(self.ctx, count, n.data_ptr(), j.data_ptr(), P.data_ptr(), out.data_ptr())
         return out
+
+    def match_moments(self, n_t, j_t, P_t):
+        mphv_match_moments(self.ctx, n_t.data_ptr(), j_t.data_ptr(), P_t.data_ptr())
 
     def exchange_maxwellian(self, dim, side, n_fl, j_fl, P_fl):
         mphv_exchange_maxwellian(self.ctx, dim, side, n_fl.data_ptr(), j_fl.data_ptr(), P_fl.data_ptr())

@@ -71,6 +71,27 @@ def test_exchange_maxwellian_matches_oracle(torch_cuda, mphv, orc, nx, dim, side
     assert np.max(np.abs(got - ref) / scale) <= TOL
 
 
+@pytest.mark.parametrize("nx,nv", [((4, 4, 1), (12, 12, 8)), ((4, 1, 4), (9, 7, 5)), ((4, 4, 1), (40, 40, 8))])
+def test_match_moments_matches_oracle(torch_cuda, mphv, orc, nx, nv):
+    torch = torch_cuda
+    from paper_2305_01487_b200 import inputs
+    w = small_workload(nx, nv, (0, 0, 0))
+    f0, _, _, _ = inputs.make_all(w)
+    sim = mphv.Vlasov.from_workload(w)
+    grid, box = orc.Grid(w.nx, w.nv, w.bc), orc.Box(w.xlo, w.xhi, w.vlo, w.vhi)
+    ns = grid.n_space
+    n, j, P = _random_moments(np.random.default_rng(33), ns)
+    ref = f0.copy()
+    orc.match_moments(ref, grid, box, n, j, P)
+    f = torch.from_numpy(f0).cuda()
+    sim.bind_f(f)
+    sim.match_moments(torch.from_numpy(n).cuda(), torch.from_numpy(j).cuda(), torch.from_numpy(P).cuda())
+    torch.cuda.synchronize()
+    got = f.cpu().numpy()
+    scale = np.maximum(np.max(np.abs(ref), axis=(3, 4, 5), keepdims=True), np.max(np.abs(f0), axis=(3, 4, 5), keepdims=True))
+    assert np.max(np.abs(got - ref) / scale) <= TOL
+
+
 def test_maxwellian_errors(torch_cuda, mphv, orc):
     w = small_workload((4, 4, 1), (8, 8, 8))
     sim = mphv.Vlasov.from_workload(w)

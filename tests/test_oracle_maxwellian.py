@@ -158,3 +158,34 @@ def test_x3_maxwellian_vlasov_state_gives_the_fluid_maxwellian(orc):
     for li, idx in enumerate([4, 5]):
         Mfl = orc.maxwellian(grid, box, n_fl[li], j_fl[:, li], P_fl[:, li]).reshape(f[:, :, idx].shape)
         assert np.max(np.abs(f[:, :, idx] - Mfl)) <= 1e-9        # f_ext - M[mom f_ext] = quadrature defect only
+
+
+def test_r18_match_moments(orc):
+    """f <- M[target] + (f - M[mom f]): the cell then carries the target moments (up to the quadrature
+    defect of the two Maxwellians), its non-Maxwellian remainder is unchanged, matching to its own
+    moments changes nothing, and matching is idempotent."""
+    grid, box, f, n_fl, j_fl, P_fl = _exchange_setup(orc, 0)
+    ns = grid.n_space
+    rng = np.random.default_rng(41)
+    tn, tj, tP = [], [], []
+    for _ in range(ns):
+        C = np.diag(0.8 + 0.5 * rng.random(3)); C[1, 2] = C[2, 1] = -0.15
+        a, b, c = _moments_from(0.6 + rng.random(), 0.4 * rng.standard_normal(3), C)
+        tn.append(a); tj.append(b); tP.append(c)
+    n_t = np.array(tn).reshape(grid.shape[:3])
+    j_t = np.array(tj).T.reshape((3,) + grid.shape[:3]).copy()
+    P_t = np.array(tP).T.reshape((6,) + grid.shape[:3]).copy()
+    f0 = f.copy()
+    n0, j0, P0 = orc.moments(f0, grid, box)
+    rem0 = f0 - orc.maxwellian(grid, box, n0.reshape(-1), j0.reshape(3, -1), P0.reshape(6, -1)).reshape(f0.shape)
+    orc.match_moments(f, grid, box, n_t, j_t, P_t)
+    n1, j1, P1 = orc.moments(f, grid, box)
+    assert np.max(np.abs(n1 - n_t)) <= 1e-7 and np.max(np.abs(j1 - j_t)) <= 1e-7 and np.max(np.abs(P1 - P_t)) <= 1e-6
+    rem1 = f - orc.maxwellian(grid, box, n_t.reshape(-1), j_t.reshape(3, -1), P_t.reshape(6, -1)).reshape(f.shape)
+    assert np.max(np.abs(rem1 - rem0)) <= 1e-15
+    g = f.copy()
+    orc.match_moments(g, grid, box, n_t, j_t, P_t)                  # idempotent up to the quadrature defect
+    assert np.max(np.abs(g - f)) <= 1e-7
+    h = f0.copy()
+    orc.match_moments(h, grid, box, n0, j0, P0)                     # own moments: nothing changes
+    assert np.max(np.abs(h - f0)) <= 1e-15
