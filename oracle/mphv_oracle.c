@@ -30,6 +30,8 @@
  * plain sweeps at B = 0, gyration closure at large angle, conservation, positivity;
  * for the ten-moment Maxwellian and the exchange of Maxwellians (R16, R17): closed
  * form, scipy's multivariate normal, moment reproduction, the sigma weights.
+ * PARITY UNPINNED for orc_match_moments (R18) beyond its own definition: Algorithm 1 of the paper is
+ * missing from PAPER.md; only the matching operation named at P:L187 is stated.
  * PARITY UNPINNED against the authors' own implementation: PAPER.md prints no
  * value of their scheme's output anywhere.
  *
