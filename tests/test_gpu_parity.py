@@ -381,3 +381,24 @@ def test_run_host_roundtrip(torch_cuda, mphv, orc):
     n_r, j_r, P_r = orc.moments(p.f_ref, p.grid, p.box)
     assert np.max(np.abs(nh.numpy() - n_r) / np.abs(n_r)) <= 1e-12
     assert np.max(np.abs(Ph.numpy()[0] - P_r[0]) / np.abs(P_r[0])) <= 1e-12
+
+
+@pytest.mark.parametrize("fusion,vmode", [(3, 0), (1, 0), (3, 1)])
+def test_step_is_bitwise_reproducible(torch_cuda, mphv, orc, fusion, vmode):
+    """Race check by determinism (compute-sanitizer is not available on the GPU pool): the fused kernels
+    recycle shared-memory ring slots and update f in place; a missing wait or barrier would show as
+    run-to-run differences. Config 1 (33.5 M cells: every SM busy, many CTAs per SM over time)."""
+    from paper_2305_01487_b200 import inputs
+    w = inputs.config(1)
+    p = Pair(torch_cuda, mphv, orc, w, fusion=fusion)
+    p.sim.set_vmode(vmode)
+    dt = 0.9 * p.dt
+    results = []
+    for _ in range(3):
+        p.f_dev.copy_(torch_cuda.from_numpy(p.f0))
+        for _ in range(2):
+            n, j, P = p.sim.step_moments(dt)
+        torch_cuda.cuda.synchronize()
+        results.append((p.f_dev.clone(), n.clone(), P.clone()))
+    for r in results[1:]:
+        assert torch_cuda.equal(r[0], results[0][0]) and torch_cuda.equal(r[1], results[0][1]) and torch_cuda.equal(r[2], results[0][2])
