@@ -25,7 +25,7 @@ namespace mphv {
 __device__ __forceinline__ double march_q(double a, double b, double c, double cx, double cy)
 {
     const double cap = b + b;
-    const double capp = (__double2hiint(cap) < 0) ? 0.0 : cap;      // max(cap, +0)
+    const double capp = b + fabs(b);                                // max(cap, +0) exactly: 2b for b >= 0, +0 for b < 0 (one DADD, no select)
     const double dp = c - b, dm = a - b;
     const double lp = (capp < dp) ? cap : dp;
     const double lm = (capp < dm) ? cap : dm;

@@ -58,7 +58,7 @@ __device__ __forceinline__ void mbar_arrive(uint64_t *bar)
 __device__ __forceinline__ double cell_q(double a, double b, double c, double c1, double nc2)
 {
     const double cap = b + b;
-    const double capp = (__double2hiint(cap) < 0) ? 0.0 : cap;      // max(cap, +0)
+    const double capp = b + fabs(b);                                // max(cap, +0) exactly: 2b for b >= 0, +0 for b < 0 (one DADD, no select)
     const double dp = c - b, dm = a - b;
     const double lp = (capp < dp) ? cap : dp;
     const double lm = (capp < dm) ? cap : dm;                        // = -L^-
