@@ -402,3 +402,25 @@ def test_step_is_bitwise_reproducible(torch_cuda, mphv, orc, fusion, vmode):
         results.append((p.f_dev.clone(), n.clone(), P.clone()))
     for r in results[1:]:
         assert torch_cuda.equal(r[0], results[0][0]) and torch_cuda.equal(r[1], results[0][1]) and torch_cuda.equal(r[2], results[0][2])
+
+
+@pytest.mark.parametrize("fusion", [0, 3])
+def test_negative_input_follows_the_formulas_as_written(torch_cuda, mphv, orc, fusion):
+    """Reading R12: f >= 0 is a precondition, but the formulas are applied as written otherwise (no
+    clamping): data with negative entries must still agree with the oracle on every kernel path."""
+    w = small_workload((12, 8, 1), (12, 8, 8), (0, 1, 0), seed_offset=6)
+    p = Pair(torch_cuda, mphv, orc, w, fusion=fusion)
+    rng = np.random.default_rng(98)
+    f = rng.uniform(-0.3, 1.0, size=w.shape) ** 3
+    f[rng.uniform(size=w.shape) < 0.2] = 0.0
+    assert (f < 0).mean() > 0.1
+    p.set_f(f)
+    for _ in range(2):
+        orc.step(p.f_ref, p.grid, p.box, w.q_over_m, p.E, p.B, p.dt * 1.5)
+        p.sim.step(p.dt * 1.5)
+    assert rel_err(p.gpu(), p.f_ref, AX_V[2]) <= 2 * TOL_SWEEP
+    p.set_f(f)
+    p.sim.set_vmode(mphv.V_BACKSUB)
+    orc.step_backsub(p.f_ref, p.grid, p.box, w.q_over_m, p.E, p.B, p.dt)
+    p.sim.step(p.dt)
+    assert rel_err(p.gpu(), p.f_ref, AX_V[2]) <= TOL_SWEEP
