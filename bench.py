@@ -146,7 +146,7 @@ def oracle_sample(w, cpu_seconds: float):
     return sub
 
 
-def time_oracle(w, steps: int, warmup: int, cpu_seconds: float):
+def time_oracle(w, steps: int, warmup: int, cpu_seconds: float, adapt: bool = False):
     """Times oracle.step + oracle.moments, as they stand, on a bounded sample of workload w."""
     import oracle
     from paper_2305_01487_b200 import inputs
@@ -155,9 +155,13 @@ def time_oracle(w, steps: int, warmup: int, cpu_seconds: float):
     dt = 0.5 * inputs.cfl_dt(sub, E, B)          # safely inside |s| < 1 on the sub-block
     grid, box = oracle.Grid(sub.nx, sub.nv, sub.bc), oracle.Box(sub.xlo, sub.xhi, sub.vlo, sub.vhi)
     f = f0.copy()
+    tw = time.perf_counter()
     for _ in range(warmup):
         oracle.step(f, grid, box, sub.q_over_m, E, B, dt)
         oracle.moments(f, grid, box)
+    tw = (time.perf_counter() - tw) / max(1, warmup)
+    if adapt and warmup and tw > 0:                              # enough steps for ~cpu_seconds of timed work
+        steps = int(min(16, max(steps, round(cpu_seconds / tw))))
     t0 = time.perf_counter()
     for _ in range(steps):
         oracle.step(f, grid, box, sub.q_over_m, E, B, dt)
@@ -354,7 +358,7 @@ def run_mphv(args, w):
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         del f0
-        line["cpu_baseline"] = {k: v for k, v in time_oracle(w, 2, 1, args.cpu_seconds).items() if k != "ms_per_step"}
+        line["cpu_baseline"] = {k: v for k, v in time_oracle(w, 2, 1, args.cpu_seconds, adapt=True).items() if k != "ms_per_step"}
 
     if rank == 0:
         print(json.dumps(line), flush=True)
