@@ -230,7 +230,7 @@ int mphv_set_vmode(mphv_ctx *ctx, int mode);
  * 2 = the whole V stage (three sweeps and the moments) in one pass over f; 3 = level 2 plus the
  * spatial sweeps S_x and S_y in one pass over f (the default, fastest measured on B200). Levels 1..3 fall back to lower-level kernels for
  * grids their kernels do not cover (nvx, nvy not multiples of 4 resp. 2, fewer than 3 velocity
- * dimensions; nx not a multiple of 4, nvel not a multiple of 8, |s| >= 1 on a periodic axis).
+ * dimensions; nx not a multiple of 4 or above 256, nvel not a multiple of 8, |s| >= 1 on a periodic axis).
  * Results agree up to fp64 rounding at every level. */
 int mphv_set_fusion(mphv_ctx *ctx, int level);
 

@@ -209,7 +209,7 @@ const int PLANE_NS = 3;                 // same for the V_vx + V_vy variant (two
 
 // The cube kernel is specialised for the velocity-plane shapes of the BASELINE.json configs
 // (40x40, 32x32: compile-time row strides) and has a generic instance for everything else.
-enum { CUBE_40 = 0, CUBE_32 = 1, CUBE_GEN = 2 };
+enum { CUBE_40 = 0, CUBE_32 = 1, CUBE_GEN = 2, CUBE_36 = 3, CUBE_16 = 4 };   // 36^3, 16^3: the paper's own velocity grids
 
 template <bool MOM> void *cube_fn(int variant)
 {
@@ -236,6 +236,8 @@ template <bool MOM> void *vstage_fn(int variant)
     switch (variant) {
     case CUBE_40: return (void *)vstage_kernel<3, MOM, 40, 40, 416, 1>;
     case CUBE_32: return (void *)vstage_kernel<2, MOM, 32, 32, 256, 2>;
+    case CUBE_36: return (void *)vstage_kernel<3, MOM, 36, 36, 352, 1>;
+    case CUBE_16: return (void *)vstage_kernel<3, MOM, 16, 16, 64, 8>;
     default:      return (void *)vstage_kernel<3, MOM, 0, 0, 512, 1>;
     }
 }
@@ -310,7 +312,7 @@ void *sxy_fn(int C, int bcx, int bcy)
     (bcy == MPHV_BC_PERIODIC ? (void *)sxy_kernel<CC, SXY_NR, BX, BC_PER, TM, MB> : (void *)sxy_kernel<CC, SXY_NR, BX, BC_OUT, TM, MB>)
 #define SXY_PICK(CC, TM, MB) \
     (bcx == MPHV_BC_PERIODIC ? SXY_ROW(CC, TM, MB, BC_PER) : bcx == MPHV_BC_OUTFLOW ? SXY_ROW(CC, TM, MB, BC_OUT) : SXY_ROW(CC, TM, MB, BC_HALO))
-    return C == 16 ? SXY_PICK(16, 512, 1) : SXY_PICK(8, 256, 2);
+    return C == 16 ? SXY_PICK(16, 512, 1) : SXY_PICK(8, 512, 1);
 #undef SXY_PICK
 #undef SXY_ROW
 }
@@ -661,7 +663,8 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
     if (grid->nv[0] % 4 == 0 && grid->nv[1] % 4 == 0 && grid->nv[2] >= 4 && grid->nv[2] % 2 == 0) {
         const int nvx = grid->nv[0], nvy = grid->nv[1], nvz = grid->nv[2];
         const int T = (nvy * (nvx / 4) + 31) / 32 * 32;
-        const int variant = (nvx == 40 && nvy == 40) ? CUBE_40 : (nvx == 32 && nvy == 32) ? CUBE_32 : CUBE_GEN;
+        const int variant = (nvx == 40 && nvy == 40) ? CUBE_40 : (nvx == 32 && nvy == 32) ? CUBE_32
+                          : (nvx == 36 && nvy == 36) ? CUBE_36 : (nvx == 16 && nvy == 16) ? CUBE_16 : CUBE_GEN;
         const size_t smem = vstage_smem_bytes(nvx, nvy, nvz, vstage_ns(variant), T);
         int max_optin = 0, per_sm = 0;
         cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
@@ -683,7 +686,7 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
         if (c->nvel % 16 == 0 && (nx / 4) * 16 <= 512) C = 16;
         else
 #endif
-        if (c->nvel % 8 == 0 && (nx / 4) * 8 <= 256) C = 8;
+        if (c->nvel % 8 == 0 && (nx / 4) * 8 <= 512) C = 8;
         if (C) {
             const int T = (nx / 4) * C;
             size_t smem = 0;

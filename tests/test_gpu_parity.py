@@ -96,7 +96,8 @@ def test_each_sweep_matches_oracle(torch_cuda, mphv, orc, nx, nv, bc, sign):
 
 
 @pytest.mark.parametrize("nx,nv,bc", SHAPES + [((4, 4, 1), (40, 40, 8), (0, 1, 0)), ((4, 4, 1), (20, 36, 4), (0, 0, 0)),
-                                            ((4, 4, 1), (4, 4, 4), (0, 1, 0)), ((4, 4, 1), (64, 8, 1), (0, 1, 0))])
+                                            ((4, 4, 1), (4, 4, 4), (0, 1, 0)), ((4, 4, 1), (64, 8, 1), (0, 1, 0)),
+                                            ((4, 4, 1), (36, 36, 6), (0, 1, 0)), ((8, 4, 1), (16, 16, 16), (0, 1, 0))])
 @pytest.mark.parametrize("fusion", [0, 1, 2, 3])
 def test_full_step_and_moments_fused_and_unfused(torch_cuda, mphv, orc, nx, nv, bc, fusion):
     """mphv_step_moments (fused plane kernel vx+vy, fused vz+moments when fusion is on) against
@@ -219,6 +220,7 @@ SXY_SHAPES = [
     ((8, 6, 4), (8, 6, 4), (0, 1, 0)),
     ((64, 7, 1), (8, 4, 4), (0, 1, 0)),
     ((128, 6, 1), (4, 4, 1), (0, 0, 0)),
+    ((256, 5, 1), (4, 4, 1), (0, 1, 0)),     # nx = 256: 64-byte chunks, 512 threads
 ]
 
 
