@@ -290,6 +290,7 @@ int launch_vstage(mphv_ctx *c, double dt, double *n, double *j, double *P)
     a.E = c->E; a.B = c->B;
     a.n = n; a.j = j; a.P = P;
     a.dV = c->dv[0] * c->dv[1] * c->dv[2];
+    a.sixth = 1.0 / 6.0;
     a.g = c->gd;
     Timed tm(c, n ? SLOT_VCUBE_MOM : SLOT_VCUBE, (n ? 56.0 : 48.0) * (double)c->nf);
     void *fn = n ? vstage_fn<true>(c->vs_variant) : vstage_fn<false>(c->vs_variant);

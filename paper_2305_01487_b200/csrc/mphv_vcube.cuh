@@ -43,6 +43,7 @@ struct CubeArgs {
     const double *E, *B;
     double *n, *j, *P;      // MOM only
     double dV;
+    double sixth;           // 1/6 as a constant-bank operand
     GridDev g;
 };
 

@@ -28,6 +28,14 @@ __device__ __forceinline__ void courant_poly(double s, double &c1, double &nc2)
     c1 = (om * (2.0 - fr)) * (1.0 / 6.0);
     nc2 = (om * (1.0 + fr)) * (-1.0 / 6.0);
 }
+// the same with 1/6 handed in from the kernel parameters (a constant-bank operand: no immediate moves) and
+// t = 1 - |s| reused: c1 = (t/6)(1 + t), -c2 = -(t/6)(2 - t)
+__device__ __forceinline__ void courant_poly6(double s, double sixth, double &c1, double &nc2)
+{
+    const double t = 1.0 - fabs(s), u = t * sixth;
+    c1 = u * (1.0 + t);
+    nc2 = -u * (2.0 - t);
+}
 
 template <int NS, bool MOM, int NVX, int NVY, int TMAX, int MINB>
 __global__ void __launch_bounds__(TMAX, MINB)
@@ -163,7 +171,7 @@ vstage_kernel(const CubeArgs p)
                     const double w[8] = { l.x, l.y, o0.x, o0.y, o1.x, o1.y, r.x, r.y };
                     const double s = fma(vzt[2 * jA + h], bx, ax);
                     double c1, nc2, o[4];
-                    courant_poly(s, c1, nc2);
+                    courant_poly6(s, p.sixth, c1, nc2);
                     remap4(w, s, c1, nc2, xlo_wall, xhi_wall, o);
                     double2 *xo = reinterpret_cast<double2 *>(xdst + h * xcells);
                     xo[0] = make_double2(o[0], o[1]);
@@ -210,7 +218,7 @@ vstage_kernel(const CubeArgs p)
                 const int jz = 2 * jB + h;
                 const double s = fma(vzt[jz], by, ay);
                 double c1, nc2, nw[4];
-                courant_poly(s, c1, nc2);
+                courant_poly6(s, p.sixth, c1, nc2);
                 // the 7-row window starts one row later for s < 0: lanes of either sign run the same code
                 const bool pos = __double2hiint(s) >= 0;
                 const double *xi = xsrc + h * xcells;
