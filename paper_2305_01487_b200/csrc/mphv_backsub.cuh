@@ -98,6 +98,34 @@ __device__ __forceinline__ double bs_face_flux(double w0, double w1, double w2, 
     return face_flux(ps ? w0 : w3, ps ? w1 : w2, ps ? w2 : w1, s, c1, c2);
 }
 
+// VEC faces of one march step. The face displacement is affine along the pencil, so the sign of s rarely
+// changes inside a warp: where every lane agrees the upwind triple needs no selects.
+template <int VEC>
+__device__ __forceinline__ void bs_face_fluxes(const double *w0, const double *w1, const double *w2, const double *w3,
+                                               const double *s, double *ph)
+{
+    bool allpos = true, allneg = true;
+#pragma unroll
+    for (int l = 0; l < VEC; ++l) { const bool ps = __double2hiint(s[l]) >= 0; allpos = allpos && ps; allneg = allneg && !ps; }
+    const unsigned mask = __activemask();
+    if (__all_sync(mask, allpos)) {
+#pragma unroll
+        for (int l = 0; l < VEC; ++l) {
+            const double fr = fabs(s[l]), om = 1.0 - fr;
+            ph[l] = face_flux(w0[l], w1[l], w2[l], s[l], (om * (2.0 - fr)) * (1.0 / 6.0), (om * (1.0 + fr)) * (1.0 / 6.0));
+        }
+    } else if (__all_sync(mask, allneg)) {
+#pragma unroll
+        for (int l = 0; l < VEC; ++l) {
+            const double fr = fabs(s[l]), om = 1.0 - fr;
+            ph[l] = face_flux(w3[l], w2[l], w1[l], s[l], (om * (2.0 - fr)) * (1.0 / 6.0), (om * (1.0 + fr)) * (1.0 / 6.0));
+        }
+    } else {
+#pragma unroll
+        for (int l = 0; l < VEC; ++l) ph[l] = bs_face_flux(w0[l], w1[l], w2[l], w3[l], s[l]);
+    }
+}
+
 // ---------------------------------------------------------------- strided axes vy, vz
 // f viewed as [outer][n][inner]: dim 1: outer = (cell, jz), inner = nvx; dim 2: outer = cell, inner = nvy nvx.
 template <int VEC, int U>
@@ -159,10 +187,13 @@ bs_march_kernel(const BacksubArgs p, int dim, long long outer, int n, long long 
                 }
                 if (i + 2 + U < n) buf[u] = ldv<VEC>(base + (long long)(i + 2 + U) * inner);
                 T out;
+                double sf[VEC], phv[VEC];
+#pragma unroll
+                for (int l = 0; l < VEC; ++l) sf[l] = fma(fi, sB, sA[l]);
+                bs_face_fluxes<VEC>(w0.v, w1.v, w2.v, w3.v, sf, phv);
 #pragma unroll
                 for (int l = 0; l < VEC; ++l) {
-                    double ph = bs_face_flux(w0.v[l], w1.v[l], w2.v[l], w3.v[l], fma(fi, sB, sA[l]));
-                    if (i == n - 1) ph = 0.0;        // closed box (R7)
+                    const double ph = i == n - 1 ? 0.0 : phv[l];       // closed box (R7)
                     out.v[l] = w1.v[l] + (pl[l] - ph);
                     pl[l] = ph;
                 }
@@ -192,10 +223,20 @@ bs_vx_kernel(const BacksubArgs p, long long rows, int rows_per_cta)
     double *rowp = nullptr;
     if (active) {
         rowp = p.f + row * nvx;
+        if (CH == 1) {
 #pragma unroll
-        for (int m = 0; m < CH + 4; ++m) {
-            const int c = q * CH - 2 + m;
-            w[m] = (c >= 0 && c < nvx) ? rowp[c] : 0.0;
+            for (int m = 0; m < CH + 4; ++m) {
+                const int c = q * CH - 2 + m;
+                w[m] = (c >= 0 && c < nvx) ? rowp[c] : 0.0;
+            }
+        } else {                                     // 16-byte loads: the thread's cells and the 2 + 2 cells beside them
+            const double2 *p2 = reinterpret_cast<const double2 *>(rowp + q * CH);
+#pragma unroll
+            for (int m = 0; m < CH / 2 + 2; ++m) {
+                const bool in = (m > 0 || q > 0) && (m < CH / 2 + 1 || q + 1 < cpr);
+                const double2 t = in ? p2[m - 1] : make_double2(0.0, 0.0);
+                w[2 * m] = t.x; w[2 * m + 1] = t.y;
+            }
         }
         const long long plane = row / g.nv[1];
         const int jy = (int)(row - plane * g.nv[1]);
@@ -214,8 +255,14 @@ bs_vx_kernel(const BacksubArgs p, long long rows, int rows_per_cta)
     for (int m = 0; m <= CH; ++m) phi[m] = bs_face_flux(w[m], w[m + 1], w[m + 2], w[m + 3], fma((double)m, sB, sA));
     if (q == 0) phi[0] = 0.0;                        // closed box (R7)
     if (q == cpr - 1) phi[CH] = 0.0;
+    if (CH == 1) {
+        rowp[q] = w[2] + (phi[0] - phi[1]);
+    } else {
 #pragma unroll
-    for (int m = 0; m < CH; ++m) rowp[q * CH + m] = w[m + 2] + (phi[m] - phi[m + 1]);
+        for (int m = 0; m < CH; m += 2)
+            *reinterpret_cast<double2 *>(rowp + q * CH + m) =
+                make_double2(w[m + 2] + (phi[m] - phi[m + 1]), w[m + 3] + (phi[m + 1] - phi[m + 2]));
+    }
 }
 
 }  // namespace mphv
