@@ -14,6 +14,8 @@ X stage (mphv_pack_halo -> NCCL send/recv -> mphv_stage_x_halo: S_x with the rec
 in one pass); time = max over ranks.
 --decomp none instead runs N independent seeded problems (no exchange); --decomp halo at N = 1
 sends the spatial sweeps through the same pack / halo kernels with the block as its own neighbour.
+JSON keys beyond the contract: "e2e" = mphv_run_host (f itself crosses PCIe both ways every step);
+"e2e_resident" = mphv_step_fields_host (f resident; host E, B in and host n, j, P out every step).
 --impl reference times the CPU oracle (oracle/) on a bounded spatial sub-block of the same
 workload on the host cores; rank 0 only.
 """
@@ -355,6 +357,25 @@ def run_mphv(args, w):
                                 if halo_mode else
                                 "mphv_run_host: pinned host f -> device, full split step, moments, f and moments -> host")}
         del fh
+        if not halo_mode:
+            # coupled run, f resident: per step the host hands over E, B and gets n, j, P back
+            Eh, Bh = torch.from_numpy(E).pin_memory(), torch.from_numpy(B).pin_memory()
+            sim.step_fields_host(Eh, Bh, dt, nh, jh, Ph)            # warm-up
+            barrier()
+            t0 = time.perf_counter()
+            for _ in range(args.steps):
+                sim.step_fields_host(Eh, Bh, dt, nh, jh, Ph)
+            barrier()
+            wall = time.perf_counter() - t0
+            if world > 1:
+                t = torch.tensor([wall], dtype=torch.float64, device=dev)
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+                wall = float(t.item())
+            line["e2e_resident"] = {"value": w.n_cells * world * args.steps / wall, "unit": UNIT,
+                                    "h2d_bytes_per_step": 6 * wr.n_space * 8, "d2h_bytes_per_step": 10 * wr.n_space * 8,
+                                    "ms_per_step": 1e3 * wall / args.steps, "steps": args.steps,
+                                    "what": "mphv_step_fields_host: f stays on the device; pinned host E, B -> device, "
+                                            "set_fields, full split step, moments -> host, stream sync every step (wall clock)"}
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         del f0

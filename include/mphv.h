@@ -163,6 +163,14 @@ int mphv_step_moments(mphv_ctx *ctx, double dt, double *n_dev, double *j_dev, do
 int mphv_run_host(mphv_ctx *ctx, double *f_host, int nsteps, double dt,
                   double *n_host, double *j_host, double *P_host);
 
+/* One step of a COUPLED run with f resident on the device (the way the paper's framework drives a Vlasov
+ * model: the field solver hands over E, B, the Vlasov model hands back its moments):
+ * copies E_host, B_host ([3][nz][ny][nx] each, ideally pinned) to library-owned device memory,
+ * mphv_set_fields, mphv_step_moments(dt), copies n, j, P to n_host [ns], j_host [3 ns], P_host [6 ns] and
+ * synchronises the stream. f stays in the bound device buffer. Requires bind_f. */
+int mphv_step_fields_host(mphv_ctx *ctx, const double *E_host, const double *B_host, double dt,
+                          double *n_host, double *j_host, double *P_host);
+
 /* Sum of all entries of the bound f (device reduction, deterministic order), written to
  * *sum_dev (device, 1 double). Used for the mass checks of BJ (1e-13 relative). */
 int mphv_sum_f(mphv_ctx *ctx, double *sum_dev);

@@ -30,6 +30,7 @@ struct mphv_ctx {
     double dx[3], dv[3];
     GridDev gd;
     double amax[3];          // max |a_d| over all pencils, from the last set_fields
+    double *fld;             // device copy of host fields for mphv_step_fields_host: [3 ns] E | [3 ns] B (lazy)
     double *ws;              // device workspace: [10 ns] moments | [10 ns mom_tiles] partials | [SUM_BLOCKS] | [8]
     int mom_tiles, mom_per_tile, mom_block;   // CTA tiling of the fused V_vz + moments kernel
     int sm_count;
@@ -714,6 +715,7 @@ int mphv_destroy(mphv_ctx *c)
 {
     if (!c) return MPHV_ERR_ARG;
     if (c->ws) cudaFree(c->ws);
+    if (c->fld) cudaFree(c->fld);
     if (c->bs_K) cudaFree(c->bs_K);
     if (c->pending) { drain_timing(c, false); delete c->pending; }
     delete c;
@@ -983,6 +985,29 @@ int mphv_run_host(mphv_ctx *c, double *f_host, int nsteps, double dt, double *n_
     if (n_host) CUDA_TRY(c, cudaMemcpyAsync(n_host, mn, c->ns * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     if (j_host) CUDA_TRY(c, cudaMemcpyAsync(j_host, mj, 3 * c->ns * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     if (P_host) CUDA_TRY(c, cudaMemcpyAsync(P_host, mP, 6 * c->ns * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return MPHV_OK;
+}
+
+int mphv_step_fields_host(mphv_ctx *c, const double *E_host, const double *B_host, double dt,
+                          double *n_host, double *j_host, double *P_host)
+{
+    if (!c) return MPHV_ERR_ARG;
+    if (!E_host || !B_host || !n_host || !j_host || !P_host) { set_err(c, "a host pointer is NULL"); return MPHV_ERR_ARG; }
+    if (!c->f) { set_err(c, "f not bound (mphv_bind_f)"); return MPHV_ERR_STATE; }
+    if (!c->fld) {
+        cudaError_t e = cudaMalloc(&c->fld, 6 * c->ns * sizeof(double));
+        if (e != cudaSuccess) { c->fld = nullptr; return cuda_fail(c, e, "cudaMalloc field staging"); }
+    }
+    CUDA_TRY(c, cudaMemcpyAsync(c->fld, E_host, 3 * c->ns * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->fld + 3 * c->ns, B_host, 3 * c->ns * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+    int st = mphv_set_fields(c, c->fld, c->fld + 3 * c->ns);          // also the Courant bound of the new fields
+    if (st != MPHV_OK) return st;
+    double *mn = ws_moments(c), *mj = mn + c->ns, *mP = mn + 4 * c->ns;
+    if ((st = step_impl(c, dt, mn, mj, mP)) != MPHV_OK) return st;
+    CUDA_TRY(c, cudaMemcpyAsync(n_host, mn, c->ns * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(j_host, mj, 3 * c->ns * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(P_host, mP, 6 * c->ns * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     return MPHV_OK;
 }

@@ -24,7 +24,7 @@ OK, ERR_ARG, ERR_STATE, ERR_RANGE, ERR_CUDA, ERR_ARCH = 0, 1, 2, 3, 4, 5
 SYMBOLS = (
     "mphv_create", "mphv_destroy", "mphv_set_stream", "mphv_f_count", "mphv_space_count",
     "mphv_bind_f", "mphv_set_fields", "mphv_sweep_x", "mphv_sweep_v", "mphv_step",
-    "mphv_moments", "mphv_step_moments", "mphv_run_host", "mphv_sum_f", "mphv_launch_count",
+    "mphv_moments", "mphv_step_moments", "mphv_run_host", "mphv_step_fields_host", "mphv_sum_f", "mphv_launch_count",
     "mphv_set_fusion", "mphv_set_vmode", "mphv_maxwellian", "mphv_exchange_maxwellian", "mphv_match_moments", "mphv_strerror", "mphv_last_error",
     "mphv_set_timing", "mphv_timing_slots", "mphv_get_timing",
     "mphv_stage_x", "mphv_stage_x_halo", "mphv_stage_v", "mphv_halo_count", "mphv_pack_halo", "mphv_sweep_x_halo",
@@ -72,6 +72,7 @@ def lib() -> C.CDLL:
         "mphv_moments": (i32, [vp, vp, vp, vp]),
         "mphv_step_moments": (i32, [vp, dbl, vp, vp, vp]),
         "mphv_run_host": (i32, [vp, vp, i32, dbl, vp, vp, vp]),
+        "mphv_step_fields_host": (i32, [vp, vp, vp, dbl, vp, vp, vp]),
         "mphv_sum_f": (i32, [vp, vp]),
         "mphv_launch_count": (C.c_uint64, [vp]),
         "mphv_set_fusion": (i32, [vp, i32]),
@@ -200,6 +201,10 @@ def mphv_sweep_x_halo(ctx, dim: int, dt: float, lo_dev=None, hi_dev=None):
 
 def mphv_run_host(ctx, f_host: int, nsteps: int, dt: float, n_host=None, j_host=None, P_host=None):
     _check(ctx, lib().mphv_run_host(ctx, f_host, int(nsteps), float(dt), n_host, j_host, P_host))
+
+
+def mphv_step_fields_host(ctx, E_host: int, B_host: int, dt: float, n_host: int, j_host: int, P_host: int):
+    _check(ctx, lib().mphv_step_fields_host(ctx, E_host, B_host, float(dt), n_host, j_host, P_host))
 
 
 def mphv_sum_f(ctx, sum_dev: int):
@@ -366,6 +371,11 @@ class Vlasov:
         def hp(t):
             return None if t is None else t.data_ptr()
         mphv_run_host(self.ctx, f_host.data_ptr(), nsteps, dt, hp(n_host), hp(j_host), hp(P_host))
+
+    def step_fields_host(self, E_host, B_host, dt, n_host, j_host, P_host):
+        """Coupled step with f resident: host fields in, host moments out (CPU float64 tensors, pinned for speed)."""
+        mphv_step_fields_host(self.ctx, E_host.data_ptr(), B_host.data_ptr(), dt,
+                              n_host.data_ptr(), j_host.data_ptr(), P_host.data_ptr())
 
     @property
     def launches(self) -> int:

@@ -426,3 +426,22 @@ def test_negative_input_follows_the_formulas_as_written(torch_cuda, mphv, orc, f
     orc.step_backsub(p.f_ref, p.grid, p.box, w.q_over_m, p.E, p.B, p.dt)
     p.sim.step(p.dt)
     assert rel_err(p.gpu(), p.f_ref, AX_V[2]) <= TOL_SWEEP
+
+
+def test_step_fields_host_coupled_step(torch_cuda, mphv, orc):
+    """mphv_step_fields_host: host fields in, f resident, host moments out = oracle step + moments."""
+    torch = torch_cuda
+    w = small_workload((12, 8, 1), (8, 8, 8))
+    p = Pair(torch, mphv, orc, w)
+    Eh, Bh = torch.from_numpy(p.E).pin_memory(), torch.from_numpy(p.B).pin_memory()
+    nh = torch.empty(w.space_shape, dtype=torch.float64).pin_memory()
+    jh = torch.empty((3,) + w.space_shape, dtype=torch.float64).pin_memory()
+    Ph = torch.empty((6,) + w.space_shape, dtype=torch.float64).pin_memory()
+    for _ in range(2):
+        orc.step(p.f_ref, p.grid, p.box, w.q_over_m, p.E, p.B, p.dt)
+        p.sim.step_fields_host(Eh, Bh, p.dt, nh, jh, Ph)
+    assert rel_err(p.gpu(), p.f_ref, AX_V[2]) <= 2 * TOL_SWEEP
+    n_r, j_r, P_r = orc.moments(p.f_ref, p.grid, p.box)
+    scale = np.abs(P_r[0]) + np.abs(P_r[3]) + np.abs(P_r[5]) + np.abs(n_r)
+    for a, b in [(nh.numpy(), n_r), (jh.numpy(), j_r), (Ph.numpy(), P_r)]:
+        assert np.max(np.abs(a - b) / scale) <= 1e-12
