@@ -235,14 +235,17 @@ void *plane_fn(int variant)
 template <bool MOM> void *vstage_fn(int variant)
 {
     switch (variant) {
-    case CUBE_40: return (void *)vstage_kernel<3, MOM, 40, 40, 416, 1>;
+#ifndef MPHV_VS40_NS
+#define MPHV_VS40_NS 3
+#endif
+    case CUBE_40: return (void *)vstage_kernel<MPHV_VS40_NS, MOM, 40, 40, 416, 1>;
     case CUBE_32: return (void *)vstage_kernel<2, MOM, 32, 32, 256, 2>;
     case CUBE_36: return (void *)vstage_kernel<3, MOM, 36, 36, 352, 1>;
     case CUBE_16: return (void *)vstage_kernel<3, MOM, 16, 16, 64, 8>;
     default:      return (void *)vstage_kernel<3, MOM, 0, 0, 512, 1>;
     }
 }
-int vstage_ns(int variant) { return variant == CUBE_32 ? 2 : 3; }
+int vstage_ns(int variant) { return variant == CUBE_32 ? 2 : variant == CUBE_40 ? MPHV_VS40_NS : 3; }
 
 size_t vstage_smem_bytes(int nvx, int nvy, int nvz, int ns, int T)
 {
