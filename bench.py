@@ -54,6 +54,9 @@ def parse():
                     help="'halo' = one spatially decomposed problem with neighbour exchange (the default for N > 1; "
                          "at N = 1 the block is its own periodic neighbour), 'none' = N independent problems "
                          "(the default at N = 1)")
+    ap.add_argument("--aux", action="store_true",
+                    help="instead of the step: time the coupling kernels of SURVEY 8(f) (ten-moment Maxwellian fill, "
+                         "exchange of Maxwellians, moment matching) on the same workload and print one JSON line")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -387,11 +390,51 @@ def run_mphv(args, w):
         dist.destroy_process_group()
 
 
+def run_aux(args, w):
+    """Device times (CUDA events in the library, per launch) of mphv_maxwellian, mphv_exchange_maxwellian and
+    mphv_match_moments on workload w; algorithmic bytes: 8 per cell written (fill), 16 per boundary cell
+    (exchange: f_ext read, ghost written), 24 per cell (matching: f read for its moments, read again, written)."""
+    import torch
+    from paper_2305_01487_b200 import inputs, mphv
+    dev = torch.device("cuda", 0)
+    f0, E, B, dt = inputs.make_all(w)
+    sim = mphv.Vlasov.from_workload(w, device=dev)
+    f = torch.from_numpy(f0).to(dev)
+    sim.bind_f(f)
+    sim.set_fields(torch.from_numpy(E).to(dev), torch.from_numpy(B).to(dev))
+    n, j, P = sim.step_moments(dt)
+    ns = w.n_space
+    n1, j1, P1 = n.reshape(-1).contiguous(), j.reshape(3, -1).contiguous(), P.reshape(6, -1).contiguous()
+    out = torch.empty_like(f)
+    dim = 1 if w.nx[1] >= 4 else 0
+    plane = ns // w.nx[dim]
+    nf = torch.ones(2 * plane, dtype=torch.float64, device=dev)
+    jf = torch.zeros(6 * plane, dtype=torch.float64, device=dev)
+    Pf = torch.zeros(6, 2 * plane, dtype=torch.float64, device=dev)
+    Pf[0] = Pf[3] = Pf[5] = 1.0
+    for rep in range(2):                                  # first pass = warm-up
+        sim.set_timing(True)
+        for _ in range(args.steps):
+            sim.maxwellian(n1, j1, P1, out=out.view(ns, w.nv[2], w.nv[1], w.nv[0]))
+            sim.exchange_maxwellian(dim, 1, nf, jf, Pf)
+            sim.match_moments(n, j, P)
+        torch.cuda.synchronize()
+        t = sim.timings()
+        sim.set_timing(False)
+    kern = {k: {"ms_per_launch": round(v["ms"] / v["launches"], 4),
+                "alg_GBps": round(v["alg_bytes"] / (v["ms"] / v["launches"] * 1e-3) / 1e9, 1)} for k, v in t.items()}
+    print(json.dumps({"metric": "aux_kernels", "config": {"workload": w.name, "cells": w.n_cells,
+                      "exchange": f"axis {dim}, high end, {2 * plane} boundary cells"},
+                      "dtype": "f64", "data": "synthetic", "kernels": kern}), flush=True)
+
+
 def main():
     args = parse()
     from paper_2305_01487_b200 import inputs
     w = inputs.config(args.config)
-    if args.impl == "reference":
+    if args.aux:
+        run_aux(args, w)
+    elif args.impl == "reference":
         run_reference(args, w)
     else:
         run_mphv(args, w)

@@ -146,6 +146,16 @@ double max_courant_v(const mphv_ctx *c, int d, double dt)
     return std::fabs((c->amax[d] * dt) / c->dv[d]);   // NaN propagates
 }
 
+// threads per CTA for kernels whose threads loop over the (vy, vx) plane of one spatial cell: the smallest
+// multiple of 32 that covers the plane in the same number of rounds as 512 threads would (1600 -> 416, not 512)
+int plane_block(long long plane)
+{
+    const long long rounds = (plane + 511) / 512;
+    long long b = (plane + rounds - 1) / rounds;
+    b = (b + 31) / 32 * 32;
+    return (int)(b < 32 ? 32 : (b > 512 ? 512 : b));
+}
+
 unsigned grid_for(long long threads, int block) { return (unsigned)((threads + block - 1) / block); }
 
 // ---- launchers ---------------------------------------------------------------------------
@@ -913,9 +923,7 @@ int mphv_exchange_maxwellian(mphv_ctx *c, int dim, int side, const double *n_fl,
     a.plane = (long long)(c->ns / (size_t)c->grid.nx[dim]);
     a.sa = sstride[da]; a.sb = sstride[db]; a.sd = sstride[dim];
     a.na = c->grid.nx[da]; a.n = c->grid.nx[dim]; a.side = side; a.g = c->gd;
-    const long long plane_v = (long long)c->grid.nv[0] * c->grid.nv[1];
-    int block = 512;
-    while (block > 32 && block / 2 >= plane_v) block /= 2;
+    const int block = plane_block((long long)c->grid.nv[0] * c->grid.nv[1]);
     Timed tm(c, SLOT_EXCH, 2.0 * (double)a.plane * 16.0 * (double)c->nvel);
     exchange_kernel<<<(unsigned)(2 * a.plane), block, 0, c->stream>>>(a);
     return after_launch(c, "exchange_kernel");
@@ -928,9 +936,7 @@ int mphv_match_moments(mphv_ctx *c, const double *n_t, const double *j_t, const 
     if (!c->f) { set_err(c, "f not bound (mphv_bind_f)"); return MPHV_ERR_STATE; }
     MatchArgs a;
     a.f = c->f; a.n_t = n_t; a.j_t = j_t; a.P_t = P_t; a.g = c->gd;
-    const long long plane_v = (long long)c->grid.nv[0] * c->grid.nv[1];
-    int block = 512;
-    while (block > 32 && block / 2 >= plane_v) block /= 2;
+    const int block = plane_block((long long)c->grid.nv[0] * c->grid.nv[1]);
     Timed tm(c, SLOT_MATCH, 24.0 * (double)c->nf);
     match_kernel<<<(unsigned)c->ns, block, 0, c->stream>>>(a);
     return after_launch(c, "match_kernel");

@@ -8,7 +8,8 @@
 //   ghost_i = M[fluid data of boundary cell i] + sigma_i (f_ext - M[moments of f_ext]),
 // f_ext = the last interior cell of the column (zero-gradient extension).
 // One CTA per spatial cell; the 3x3 algebra is done once per CTA by thread 0 and broadcast through
-// shared memory, the velocity cube is streamed by all threads (8 bytes written per cell, one exp).
+// shared memory, the velocity cube is streamed by all threads along vz pencils (8 bytes written per cell;
+// the Gaussian along a pencil by a two-multiplication recurrence with exact restarts, MaxwLine).
 #pragma once
 #include "mphv_kernels.cuh"
 
@@ -53,6 +54,30 @@ __device__ __forceinline__ double maxw_eval(const MaxwCoef &m, double vx, double
     return m.norm * exp(q);
 }
 
+// A Maxwellian along one vz pencil (vx, vy fixed): q(vz) is quadratic in vz, so consecutive cells follow from
+// two multiplications, e_{k+1} = e_k r_k, r_{k+1} = r_k rho with rho = exp(2 czz dvz^2); e and r are re-evaluated
+// exactly every MAXW_RS cells, which bounds the accumulated rounding to ~(RS^2/2) ulp (4e-15) and keeps
+// underflow local. One exp per cell becomes 2/RS.
+enum { MAXW_RS = 8 };
+struct MaxwLine {
+    double a0, b, e, r, rho;
+    __device__ __forceinline__ void init(const MaxwCoef &m, double vx, double vy, double dvz)
+    {
+        const double dx = vx - m.ux, dy = vy - m.uy;
+        a0 = dx * (m.cxx * dx + m.cxy * dy) + m.cyy * dy * dy;
+        b = m.cxz * dx + m.cyz * dy;
+        rho = exp(2.0 * m.czz * dvz * dvz);
+        e = 0.0; r = 0.0;
+    }
+    __device__ __forceinline__ void restart(const MaxwCoef &m, double vz, double dvz)
+    {
+        const double dz = vz - m.uz;
+        e = m.norm * exp(a0 + dz * (b + m.czz * dz));
+        r = exp(dvz * (b + m.czz * (2.0 * dz + dvz)));
+    }
+    __device__ __forceinline__ double next() { const double v = e; e *= r; r *= rho; return v; }
+};
+
 struct MaxwArgs {
     const double *n, *j, *P;    // [count], [3][count], [6][count]
     long long count;
@@ -60,7 +85,7 @@ struct MaxwArgs {
     GridDev g;
 };
 
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(512)
 maxwellian_kernel(const MaxwArgs p)
 {
     __shared__ MaxwCoef sm;
@@ -76,8 +101,12 @@ maxwellian_kernel(const MaxwArgs p)
     for (int pos = threadIdx.x; pos < plane; pos += blockDim.x) {
         const int jy = pos / g.nv[0], jx = pos - jy * g.nv[0];
         const double vx = vcentre(g, 0, jx), vy = vcentre(g, 1, jy);
-        for (int jz = 0; jz < g.nv[2]; ++jz)
-            cube[(long long)jz * plane + pos] = m.norm > 0.0 ? maxw_eval(m, vx, vy, vcentre(g, 2, jz)) : 0.0;
+        MaxwLine ln;
+        ln.init(m, vx, vy, g.dv[2]);
+        for (int jz = 0; jz < g.nv[2]; ++jz) {
+            if (jz % MAXW_RS == 0) ln.restart(m, vcentre(g, 2, jz), g.dv[2]);
+            cube[(long long)jz * plane + pos] = m.norm > 0.0 ? ln.next() : 0.0;
+        }
     }
 }
 
@@ -119,11 +148,16 @@ exchange_kernel(const ExchArgs p)
         const int jy = pos / g.nv[0], jx = pos - jy * g.nv[0];
         const double vx = vcentre(g, 0, jx), vy = vcentre(g, 1, jy);
         double s0 = 0.0, s1 = 0.0, s2 = 0.0;
-        for (int jz = 0; jz < g.nv[2]; ++jz) {
-            const double fv = fext[(long long)jz * plane + pos];
-            const double vz = vcentre(g, 2, jz);
-            const double t = vz * fv;
-            s0 += fv; s1 += t; s2 = fma(vz, t, s2);
+        for (int j0 = 0; j0 < g.nv[2]; j0 += 8) {
+            double fv[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) fv[u] = j0 + u < g.nv[2] ? fext[(long long)(j0 + u) * plane + pos] : 0.0;
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const double vz = vcentre(g, 2, j0 + u);
+                const double t = vz * fv[u];
+                s0 += fv[u]; s1 += t; s2 = fma(vz, t, s2);
+            }
         }
         const double x0 = vx * s0, y0 = vy * s0;
         m[0] += s0;
@@ -145,11 +179,20 @@ exchange_kernel(const ExchArgs p)
     for (int pos = threadIdx.x; pos < plane; pos += blockDim.x) {
         const int jy = pos / g.nv[0], jx = pos - jy * g.nv[0];
         const double vx = vcentre(g, 0, jx), vy = vcentre(g, 1, jy);
-        for (int jz = 0; jz < g.nv[2]; ++jz) {
-            const double vz = vcentre(g, 2, jz);
-            const double a = mfl.norm > 0.0 ? maxw_eval(mfl, vx, vy, vz) : 0.0;
-            const double b = mex.norm > 0.0 ? maxw_eval(mex, vx, vy, vz) : 0.0;
-            dst[(long long)jz * plane + pos] = a + sigma * (fext[(long long)jz * plane + pos] - b);
+        MaxwLine la, lb;
+        la.init(mfl, vx, vy, g.dv[2]); lb.init(mex, vx, vy, g.dv[2]);
+        for (int j0 = 0; j0 < g.nv[2]; j0 += MAXW_RS) {
+            const double vz = vcentre(g, 2, j0);
+            la.restart(mfl, vz, g.dv[2]); lb.restart(mex, vz, g.dv[2]);
+            double fv[MAXW_RS];
+#pragma unroll
+            for (int u = 0; u < MAXW_RS; ++u) fv[u] = j0 + u < g.nv[2] ? fext[(long long)(j0 + u) * plane + pos] : 0.0;
+#pragma unroll
+            for (int u = 0; u < MAXW_RS; ++u) {
+                const double a = mfl.norm > 0.0 ? la.next() : 0.0;
+                const double b = mex.norm > 0.0 ? lb.next() : 0.0;
+                if (j0 + u < g.nv[2]) dst[(long long)(j0 + u) * plane + pos] = a + sigma * (fv[u] - b);
+            }
         }
     }
 }
@@ -179,11 +222,16 @@ match_kernel(const MatchArgs p)
         const int jy = pos / g.nv[0], jx = pos - jy * g.nv[0];
         const double vx = vcentre(g, 0, jx), vy = vcentre(g, 1, jy);
         double s0 = 0.0, s1 = 0.0, s2 = 0.0;
-        for (int jz = 0; jz < g.nv[2]; ++jz) {
-            const double fv = cube[(long long)jz * plane + pos];
-            const double vz = vcentre(g, 2, jz);
-            const double t = vz * fv;
-            s0 += fv; s1 += t; s2 = fma(vz, t, s2);
+        for (int j0 = 0; j0 < g.nv[2]; j0 += 8) {
+            double fv[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) fv[u] = j0 + u < g.nv[2] ? cube[(long long)(j0 + u) * plane + pos] : 0.0;
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const double vz = vcentre(g, 2, j0 + u);
+                const double t = vz * fv[u];
+                s0 += fv[u]; s1 += t; s2 = fma(vz, t, s2);
+            }
         }
         const double x0 = vx * s0, y0 = vy * s0;
         m[0] += s0;
@@ -205,12 +253,20 @@ match_kernel(const MatchArgs p)
     for (int pos = threadIdx.x; pos < plane; pos += blockDim.x) {
         const int jy = pos / g.nv[0], jx = pos - jy * g.nv[0];
         const double vx = vcentre(g, 0, jx), vy = vcentre(g, 1, jy);
-        for (int jz = 0; jz < g.nv[2]; ++jz) {
-            const double vz = vcentre(g, 2, jz);
-            const double a = mt.norm > 0.0 ? maxw_eval(mt, vx, vy, vz) : 0.0;
-            const double b = mf.norm > 0.0 ? maxw_eval(mf, vx, vy, vz) : 0.0;
-            double *q = cube + (long long)jz * plane + pos;
-            *q = a + (*q - b);
+        MaxwLine la, lb;
+        la.init(mt, vx, vy, g.dv[2]); lb.init(mf, vx, vy, g.dv[2]);
+        for (int j0 = 0; j0 < g.nv[2]; j0 += MAXW_RS) {
+            const double vz = vcentre(g, 2, j0);
+            la.restart(mt, vz, g.dv[2]); lb.restart(mf, vz, g.dv[2]);
+            double fv[MAXW_RS];
+#pragma unroll
+            for (int u = 0; u < MAXW_RS; ++u) fv[u] = j0 + u < g.nv[2] ? cube[(long long)(j0 + u) * plane + pos] : 0.0;
+#pragma unroll
+            for (int u = 0; u < MAXW_RS; ++u) {
+                const double a = mt.norm > 0.0 ? la.next() : 0.0;
+                const double b = mf.norm > 0.0 ? lb.next() : 0.0;
+                if (j0 + u < g.nv[2]) cube[(long long)(j0 + u) * plane + pos] = a + (fv[u] - b);
+            }
         }
     }
 }
