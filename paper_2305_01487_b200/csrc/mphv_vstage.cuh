@@ -144,7 +144,10 @@ vstage_kernel(const CubeArgs p)
     int jB = 0, cellB = 0;                           // (cell, pair in cube) of pair i-1
     double *outp = stream0 + (size_t)r0 * nvx + jx;  // plane 0 of the cube of stage B, this thread's first cell
 
-    for (int i = 0; i <= K2; ++i) {
+    // One pipeline iteration: stage A of pair i, stage B of pair i-1. FIRST / LAST: pair i-1 is the first /
+    // last pair of its cube (compile-time, so the 18 of 20 iterations in between carry no cube-boundary code).
+    auto iter = [&](auto first_tag, auto last_tag, const int i) {
+        constexpr bool FIRST = decltype(first_tag)::value, LAST = decltype(last_tag)::value;
         // ================= stage A: V_vx of planes 2i, 2i+1
         if (i < K2) {
             if (jA == 0) {                           // new cube: a_x = qm (E_x + vy B_z - vz B_y)
@@ -183,7 +186,7 @@ vstage_kernel(const CubeArgs p)
             if (slotA == 0) parA ^= 1u;
             if (++jA == hz) { jA = 0; ++cellA; }
         }
-        if (i == 0) continue;
+        if (i == 0) return;
         // ================= stage B: V_vy of planes 2(i-1), 2(i-1)+1, two V_vz march steps, moments
         const int ib = i - 1;
         mbar_wait(&bars[NS + (ib & 1)], (uint32_t)((ib >> 1) & 1));
@@ -192,7 +195,7 @@ vstage_kernel(const CubeArgs p)
             bulk_load(ring + (size_t)slotB * 2 * cells, stream0 + (size_t)(ib + NS) * 2 * cells, pair_bytes, &bars[slotB]);
         }
         slotB = slotB + 1 == NS ? 0 : slotB + 1;
-        if (jB == 0) {                               // new cube
+        if (FIRST) {                                 // new cube
             const long long c = c_begin + cellB;
             const double Ey = __ldg(p.E + p.ns + c), Ez = __ldg(p.E + 2 * p.ns + c);
             const double Bx = __ldg(p.B + c), By = __ldg(p.B + p.ns + c), Bz = __ldg(p.B + 2 * p.ns + c);
@@ -233,7 +236,7 @@ vstage_kernel(const CubeArgs p)
                 if (yhi_wall) q[4] = 0.0;
 #pragma unroll
                 for (int r = 0; r < 4; ++r) nw[r] = fma(s, q[r] - q[r + 1], xi[(r + 2) * nvx]);
-                if (jB == 0) {
+                if (FIRST) {
                     if (h == 0) {
 #pragma unroll
                         for (int m = 0; m < 4; ++m) G0[m] = nw[m];       // g_0
@@ -253,7 +256,7 @@ vstage_kernel(const CubeArgs p)
                     outp += cells;
                 }
             }
-            if (jB == hz - 1) {                      // drain: the two ghost planes behind the high wall are empty
+            if (LAST) {                              // drain: the two ghost planes behind the high wall are empty
                 const double zero[4] = { 0.0, 0.0, 0.0, 0.0 };
                 vz_step(M1(), zero, vzt[nvz - 2], outp);
                 outp += cells;
@@ -261,7 +264,7 @@ vstage_kernel(const CubeArgs p)
                 outp += cells;
             }
         }
-        if (jB == hz - 1) {
+        if (LAST) {
             if (MOM) {
                 double mom[10];
 #pragma unroll
@@ -291,6 +294,14 @@ vstage_kernel(const CubeArgs p)
         } else {
             ++jB;
         }
+    };
+    struct No { enum { value = 0 }; }; struct Yes { enum { value = 1 }; };
+    iter(No(), No(), 0);
+    int i = 1;
+    for (int cell = 0; cell < ncell; ++cell) {
+        iter(Yes(), No(), i++);
+        for (int j = 1; j < hz - 1; ++j) iter(No(), No(), i++);
+        iter(No(), Yes(), i++);
     }
 }
 
