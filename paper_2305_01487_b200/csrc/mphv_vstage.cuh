@@ -146,11 +146,13 @@ vstage_kernel(const CubeArgs p)
 
     // One pipeline iteration: stage A of pair i, stage B of pair i-1. FIRST / LAST: pair i-1 is the first /
     // last pair of its cube (compile-time, so the 18 of 20 iterations in between carry no cube-boundary code).
-    auto iter = [&](auto first_tag, auto last_tag, const int i) {
+    // AFIRST: pair i is the first of its cube; HASA: pair i exists (false only in the final call).
+    auto iter = [&](auto first_tag, auto last_tag, auto afirst_tag, auto hasa_tag, const int i) {
         constexpr bool FIRST = decltype(first_tag)::value, LAST = decltype(last_tag)::value;
+        constexpr bool AFIRST = decltype(afirst_tag)::value, HASA = decltype(hasa_tag)::value;
         // ================= stage A: V_vx of planes 2i, 2i+1
-        if (i < K2) {
-            if (jA == 0) {                           // new cube: a_x = qm (E_x + vy B_z - vz B_y)
+        if (HASA) {
+            if (AFIRST) {                            // new cube: a_x = qm (E_x + vy B_z - vz B_y)
                 const long long c = c_begin + cellA;
                 const double Ex = __ldg(p.E + c), By = __ldg(p.B + p.ns + c), Bz = __ldg(p.B + 2 * p.ns + c);
                 ax = (p.g.qm * (Ex + vy_row * Bz)) * dtdvx;
@@ -296,12 +298,13 @@ vstage_kernel(const CubeArgs p)
         }
     };
     struct No { enum { value = 0 }; }; struct Yes { enum { value = 1 }; };
-    iter(No(), No(), 0);
+    iter(No(), No(), Yes(), Yes(), 0);
     int i = 1;
     for (int cell = 0; cell < ncell; ++cell) {
-        iter(Yes(), No(), i++);
-        for (int j = 1; j < hz - 1; ++j) iter(No(), No(), i++);
-        iter(No(), Yes(), i++);
+        iter(Yes(), No(), No(), Yes(), i++);
+        for (int j = 1; j < hz - 1; ++j) iter(No(), No(), No(), Yes(), i++);
+        if (cell + 1 < ncell) iter(No(), Yes(), Yes(), Yes(), i++);
+        else                  iter(No(), Yes(), No(), No(), i++);
     }
 }
 
