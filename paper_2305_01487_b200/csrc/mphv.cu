@@ -8,6 +8,7 @@
 #include "mphv_vstage.cuh"
 #include "mphv_sxy.cuh"
 #include "mphv_backsub.cuh"
+#include "mphv_vstage_bs.cuh"
 #include "mphv_maxwell.cuh"
 
 #include <cmath>
@@ -35,7 +36,7 @@ struct mphv_ctx {
     int mom_tiles, mom_per_tile, mom_block;   // CTA tiling of the fused V_vz + moments kernel
     int sm_count;
     int vxy_T, vxy_grid; size_t vxy_smem;     // fused V_vx + V_vy plane kernel launch shape (0 = unsupported)
-    int vs_T, vs_grid, vs_variant; size_t vs_smem;   // second-generation whole-V-stage kernel (T = 0: unsupported)
+    int vs_T, vs_grid, vs_variant, vs_bs; size_t vs_smem;   // second-generation whole-V-stage kernel (T = 0: unsupported)
     int sxy_T, sxy_C; size_t sxy_smem;               // fused S_x + S_y kernel (T = 0: unsupported)
     int cube_T, cube_grid, cube_variant, plane_grid; size_t cube_smem, plane_smem;  // whole-V-stage cube kernel launch shape (T = 0: unsupported)
     int vmode;                                       // 0 plain V sweeps, 1 backsubstitution
@@ -255,6 +256,16 @@ template <bool MOM> void *vstage_fn(int variant)
     default:      return (void *)vstage_kernel<3, MOM, 0, 0, 512, 1>;
     }
 }
+template <bool MOM> void *vstage_bs_fn(int variant)
+{
+    switch (variant) {
+    case CUBE_40: return (void *)vstage_bs_kernel<MPHV_VS40_NS, MOM, 40, 40, 416, 1>;
+    case CUBE_32: return (void *)vstage_bs_kernel<2, MOM, 32, 32, 256, 2>;
+    case CUBE_36: return (void *)vstage_bs_kernel<3, MOM, 36, 36, 352, 1>;
+    case CUBE_16: return (void *)vstage_bs_kernel<3, MOM, 16, 16, 64, 8>;
+    default:      return (void *)vstage_bs_kernel<3, MOM, 0, 0, 512, 1>;
+    }
+}
 int vstage_ns(int variant) { return variant == CUBE_32 ? 2 : variant == CUBE_40 ? MPHV_VS40_NS : 3; }
 
 size_t vstage_smem_bytes(int nvx, int nvy, int nvz, int ns, int T)
@@ -293,7 +304,7 @@ int launch_vcube(mphv_ctx *c, double dt, bool with_vz, double *n, double *j, dou
 }
 
 // V_vx, V_vy, V_vz (+ moments if n != NULL) in one pass over f, two planes per pipeline iteration
-int launch_vstage(mphv_ctx *c, double dt, double *n, double *j, double *P)
+int launch_vstage(mphv_ctx *c, double dt, double *n, double *j, double *P, bool backsub = false)
 {
     CubeArgs a;
     std::memset(&a, 0, sizeof a);
@@ -307,7 +318,9 @@ int launch_vstage(mphv_ctx *c, double dt, double *n, double *j, double *P)
     a.sixth = 1.0 / 6.0;
     a.g = c->gd;
     Timed tm(c, n ? SLOT_VCUBE_MOM : SLOT_VCUBE, (n ? 56.0 : 48.0) * (double)c->nf);
-    void *fn = n ? vstage_fn<true>(c->vs_variant) : vstage_fn<false>(c->vs_variant);
+    a.K = backsub ? c->bs_K : nullptr;
+    void *fn = backsub ? (n ? vstage_bs_fn<true>(c->vs_variant) : vstage_bs_fn<false>(c->vs_variant))
+                       : (n ? vstage_fn<true>(c->vs_variant) : vstage_fn<false>(c->vs_variant));
     void *args[] = { &a };
     cudaError_t e = cudaLaunchKernel(fn, dim3((unsigned)c->vs_grid), dim3((unsigned)c->vs_T), args, c->vs_smem, c->stream);
     if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(c, e, "vstage_kernel launch"); }
@@ -493,6 +506,7 @@ int do_v_stage(mphv_ctx *c, double dt, double *n, double *j, double *P)
 {
     int st;
     const bool ax = c->grid.nv[0] > 1, ay = c->grid.nv[1] > 1, az = c->grid.nv[2] > 1;
+    if (c->vmode && c->fusion >= 2 && c->vs_T > 0 && c->vs_bs) return launch_vstage(c, dt, n, j, P, true);
     if (c->vmode) {                                  // backsubstitution: three face-displaced sweeps, then the moments
         for (int d = 0; d < 3; ++d)
             if ((st = do_sweep_v_backsub(c, d)) != MPHV_OK) return st;
@@ -690,6 +704,8 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
             long long g = (long long)per_sm * c->sm_count;
             if (g > (long long)c->ns) g = (long long)c->ns;
             c->vs_T = T; c->vs_smem = smem; c->vs_grid = (int)g; c->vs_variant = variant;
+            c->vs_bs = cudaFuncSetAttribute(vstage_bs_fn<true>(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess &&
+                       cudaFuncSetAttribute(vstage_bs_fn<false>(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess;
         }
         cudaGetLastError();
     }

@@ -44,6 +44,7 @@ struct CubeArgs {
     double *n, *j, *P;      // MOM only
     double dV;
     double sixth;           // 1/6 as a constant-bank operand
+    const double *K;        // backsubstitution mode: [ns][12] face-displacement coefficients (mphv_backsub.cuh)
     GridDev g;
 };
 
