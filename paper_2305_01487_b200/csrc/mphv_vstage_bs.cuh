@@ -86,11 +86,16 @@ vstage_bs_kernel(const CubeArgs p)
     // no flux (R7).
     auto vz_step = [&](auto mode_tag, const double (&nw)[4], double fi, double wz, double *po) {
         constexpr int MODE = decltype(mode_tag)::value;
-        double o[4];
+        double o[4], phv[4] = { 0.0, 0.0, 0.0, 0.0 };
+        if (MODE != 2) {
+            double sf[4];
+#pragma unroll
+            for (int m = 0; m < 4; ++m) sf[m] = fma(fi, sBz, zsp[m * blockDim.x]);
+            bs_face_fluxes<4>(W0, W1, W2, nw, sf, phv);
+        }
 #pragma unroll
         for (int m = 0; m < 4; ++m) {
-            double ph = 0.0;
-            if (MODE != 2) ph = bs_face_flux(W0[m], W1[m], W2[m], nw[m], fma(fi, sBz, zsp[m * blockDim.x]));
+            const double ph = phv[m];
             o[m] = W1[m] + (PL[m] - ph);
             PL[m] = ph;
             W0[m] = W1[m]; W1[m] = W2[m]; W2[m] = nw[m];
