@@ -201,8 +201,28 @@ vstage_bs_kernel(const CubeArgs p)
                 double w[8], phi[5], nw[4];
 #pragma unroll
                 for (int r = 0; r < 8; ++r) w[r] = xi[r * nvx];
+                {   // the faces of a warp almost always move the same way: select-free upwind paths
+                    const double s4 = fma(4.0, sBy, s0);
+                    const bool apos = __double2hiint(s0) >= 0 && __double2hiint(s4) >= 0;
+                    const bool aneg = __double2hiint(s0) < 0 && __double2hiint(s4) < 0;
+                    const unsigned mask = __activemask();
+                    if (__all_sync(mask, apos)) {
 #pragma unroll
-                for (int m = 0; m < 5; ++m) phi[m] = bs_face_flux(w[m], w[m + 1], w[m + 2], w[m + 3], fma((double)m, sBy, s0));
+                        for (int m = 0; m < 5; ++m) {
+                            const double sm = fma((double)m, sBy, s0), fr = fabs(sm), om = 1.0 - fr;
+                            phi[m] = face_flux(w[m], w[m + 1], w[m + 2], sm, (om * (2.0 - fr)) * (1.0 / 6.0), (om * (1.0 + fr)) * (1.0 / 6.0));
+                        }
+                    } else if (__all_sync(mask, aneg)) {
+#pragma unroll
+                        for (int m = 0; m < 5; ++m) {
+                            const double sm = fma((double)m, sBy, s0), fr = fabs(sm), om = 1.0 - fr;
+                            phi[m] = face_flux(w[m + 3], w[m + 2], w[m + 1], sm, (om * (2.0 - fr)) * (1.0 / 6.0), (om * (1.0 + fr)) * (1.0 / 6.0));
+                        }
+                    } else {
+#pragma unroll
+                        for (int m = 0; m < 5; ++m) phi[m] = bs_face_flux(w[m], w[m + 1], w[m + 2], w[m + 3], fma((double)m, sBy, s0));
+                    }
+                }
                 if (ylo_wall) phi[0] = 0.0;          // closed box (R7): the wall faces carry no flux
                 if (yhi_wall) phi[4] = 0.0;
 #pragma unroll
