@@ -106,3 +106,24 @@ def test_backsub_errors(torch_cuda, mphv, orc):
     with pytest.raises(mphv.MphvError) as e:
         sim2.set_vmode(mphv.V_BACKSUB)
     assert e.value.code == mphv.ERR_ARG
+
+
+def test_fused_backsub_kernel_is_the_one_that_runs(torch_cuda, mphv, orc):
+    """At fusion level >= 2 the backsubstituted V stage is ONE kernel (vstage_bs_kernel) where the grid allows:
+    stage_v = 1 launch (after the first call with this dt, which also runs the coefficient kernel)."""
+    w = small_workload((4, 4, 1), (32, 32, 8), (0, 1, 0))
+    p = Pair(torch_cuda, mphv, orc, w, fusion=3)
+    p.sim.set_vmode(mphv.V_BACKSUB)
+    p.sim.stage_v(p.dt)
+    n0 = p.sim.launches
+    mom = p.sim.alloc_moments()
+    p.sim.stage_v(p.dt, mom)
+    assert p.sim.launches - n0 == 1
+    for _ in range(2):
+        for d in range(3):
+            orc.sweep_v_backsub(p.f_ref, p.grid, p.box, w.q_over_m, p.E, p.B, d, p.dt)
+    assert rel_err(p.gpu(), p.f_ref, AX_V[2]) <= 2 * TOL_SWEEP
+    p.sim.set_fusion(0)
+    n0 = p.sim.launches
+    p.sim.stage_v(p.dt, mom)
+    assert p.sim.launches - n0 == 4, "three sweep kernels and the moments"
