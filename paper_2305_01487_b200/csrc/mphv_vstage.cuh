@@ -125,7 +125,7 @@ vstage_kernel(const CubeArgs p)
             o[m] = fma(zs, pos ? E[m] : en, G0[m]);
             Q[m] = qn; E[m] = en;
             G0[m] = G1[m]; G1[m] = nw[m];
-            po[m * nvx] = o[m];
+            __stcs(po + m * nvx, o[m]);              // streaming store
         }
         if (MOM) {
             const double p0 = (o[0] + o[1]) + (o[2] + o[3]);
