@@ -99,7 +99,7 @@ vstage_bs_kernel(const CubeArgs p)
             o[m] = W1[m] + (PL[m] - ph);
             PL[m] = ph;
             W0[m] = W1[m]; W1[m] = W2[m]; W2[m] = nw[m];
-            po[m * nvx] = o[m];
+            __stcs(po + m * nvx, o[m]);              // streaming store
         }
         if (MOM) {
             const double p0 = (o[0] + o[1]) + (o[2] + o[3]);
