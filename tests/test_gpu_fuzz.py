@@ -1,0 +1,58 @@
+"""Randomised parity: seeded random grids (2-D and 3-D, extents that do and do not fit the fused kernels,
+the paper's 36^3 / 40^3 / 16^3 velocity planes), boundary conditions, sign of q/m and dt, fusion level and
+V-stage mode; two steps + moments against the oracle, element by element."""
+import numpy as np
+import pytest
+
+from parity_util import local_scale
+from test_gpu_parity import torch_cuda, mphv  # noqa: F401
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("seed", [11, 12, 13])
+def test_random_configurations_match_the_oracle(torch_cuda, mphv, orc, seed):
+    torch = torch_cuda
+    from paper_2305_01487_b200 import inputs
+    rng = np.random.default_rng(seed)
+    done = 0
+    while done < 16:
+        three = rng.random() < 0.25
+        nx = (int(rng.choice([4, 8, 12, 16, 20, 32])), int(rng.choice([4, 5, 6, 9, 16])), int(rng.choice([4, 6])) if three else 1)
+        nv = (int(rng.choice([4, 8, 12, 16, 20, 36, 40])), int(rng.choice([4, 8, 12, 16, 36, 40])), int(rng.choice([4, 6, 8, 10])))
+        if np.prod(nx) * np.prod(nv) > 3e6:
+            continue
+        bc = (int(rng.integers(0, 2)), int(rng.integers(0, 2)), int(rng.integers(0, 2)) if three else 0)
+        fusion, vmode = int(rng.integers(0, 4)), int(rng.integers(0, 2))
+        w = inputs.Workload(name="fuzz", index=1, kind="harris3d" if three else "harris2d", nx=nx, nv=nv, bc=bc,
+                            xlo=(0.0, -6.4, 0.0), xhi=(25.6, 6.4, 12.8), vlo=(-5.0,) * 3, vhi=(5.0,) * 3, steps=2,
+                            seed_offset=100 * seed + done, q_over_m=float(rng.choice([1.0, -3.0])))
+        f0, E, B, dt = inputs.make_all(w)
+        dt *= float(rng.choice([1.3, -1.3, 0.6]))
+        grid, box = orc.Grid(w.nx, w.nv, w.bc), orc.Box(w.xlo, w.xhi, w.vlo, w.vhi)
+        ref = f0.copy()
+        try:
+            for _ in range(2):
+                (orc.step_backsub if vmode else orc.step)(ref, grid, box, w.q_over_m, E, B, dt)
+        except ValueError:
+            continue                                    # the oracle refuses |s| >= 1: not a parity case
+        sim = mphv.Vlasov.from_workload(w)
+        sim.set_fusion(fusion)
+        sim.set_vmode(vmode)
+        f = torch.from_numpy(f0).cuda()
+        sim.bind_f(f)
+        sim.set_fields(torch.from_numpy(E).cuda(), torch.from_numpy(B).cuda())
+        for _ in range(2):
+            n, j, P = sim.step_moments(dt)
+        torch.cuda.synchronize()
+        got = f.cpu().numpy()
+        scale = np.abs(ref)
+        for ax in (3, 4, 5):
+            scale = local_scale(scale, ax)
+        tag = f"nx {nx} nv {nv} bc {bc} fusion {fusion} vmode {vmode}"
+        assert np.max(np.abs(got - ref) / np.maximum(scale, 1e-300)) <= 2e-12, tag
+        n_r, j_r, P_r = orc.moments(ref, grid, box)
+        sc = np.abs(P_r[0]) + np.abs(P_r[3]) + np.abs(P_r[5]) + np.abs(n_r)
+        for a, b in [(n, n_r), (j, j_r), (P, P_r)]:
+            assert np.max(np.abs(a.cpu().numpy() - b) / sc) <= 1e-12, tag
+        done += 1
