@@ -102,7 +102,7 @@ vstage_kernel(const CubeArgs p)
     // s and the coefficients of lim(g_{j+1}-g_j), lim(g_{j-1}-g_j) live in zsm, zc
     double2 *const zcp = zc + tid;                   // (shared memory, written and read by this thread only)
     double *const zsp = zsm + tid;
-    double G0[4], G1[4], Q[4], E[4];                 // g_i, g_{i+1}, Q_i, E_i = Q_{i-1} - Q_i
+    double G0[4], G1[4], Q[4], E[4];                 // the two newest planes (G0: even, G1: odd), Q_i, E_i = Q_{i-1} - Q_i
     double P0 = 0.0, Q1 = 0.0, Q2 = 0.0, Z1 = 0.0, Z2 = 0.0, ZQ = 0.0;   // moment sums (see header)
 #pragma unroll
     for (int m = 0; m < 4; ++m) { G0[m] = G1[m] = Q[m] = E[m] = 0.0; }
@@ -110,7 +110,8 @@ vstage_kernel(const CubeArgs p)
     // One march step for the 4 pencils: nw = g_{i+2} arrives, Q_{i+1} is formed, cell i is finished
     // and stored to plane i (po). MODE 0: interior; 1: i = nvz-2 (Q_{i+1} sits in front of the high
     // wall); 2: i = nvz-1 (Q_{i+1} is the ghost cell behind it). Closed box, R7.
-    auto vz_step = [&](auto mode_tag, const double (&nw)[4], double wz, double *po) {
+    // (GA, GB) = (g_i, g_{i+1}) on entry; GA becomes g_{i+2} (the caller alternates the two windows: no rotation)
+    auto vz_step = [&](auto mode_tag, double (&GA)[4], double (&GB)[4], const double (&nw)[4], double wz, double *po) {
         constexpr int MODE = decltype(mode_tag)::value;
         double o[4];
 #pragma unroll
@@ -118,13 +119,13 @@ vstage_kernel(const CubeArgs p)
             const double zs = zsp[m * blockDim.x];
             const bool pos = __double2hiint(zs) >= 0;
             const double2 zxy = zcp[m * blockDim.x];
-            double qn = march_q(G0[m], G1[m], nw[m], zxy.x, zxy.y);
+            double qn = march_q(GA[m], GB[m], nw[m], zxy.x, zxy.y);
             if (MODE == 1 && pos) qn = 0.0;
             if (MODE == 2 && !pos) qn = 0.0;
             const double en = Q[m] - qn;
-            o[m] = fma(zs, pos ? E[m] : en, G0[m]);
+            o[m] = fma(zs, pos ? E[m] : en, GA[m]);
             Q[m] = qn; E[m] = en;
-            G0[m] = G1[m]; G1[m] = nw[m];
+            GA[m] = nw[m];
             __stcs(po + m * nvx, o[m]);              // streaming store
         }
         if (MOM) {
@@ -254,15 +255,16 @@ vstage_kernel(const CubeArgs p)
                         }
                     }
                 } else {
-                    vz_step(M0(), nw, vzt[jz - 2], outp);
+                    if (h == 0) vz_step(M0(), G0, G1, nw, vzt[jz - 2], outp);
+                    else        vz_step(M0(), G1, G0, nw, vzt[jz - 2], outp);
                     outp += cells;
                 }
             }
             if (LAST) {                              // drain: the two ghost planes behind the high wall are empty
                 const double zero[4] = { 0.0, 0.0, 0.0, 0.0 };
-                vz_step(M1(), zero, vzt[nvz - 2], outp);
+                vz_step(M1(), G0, G1, zero, vzt[nvz - 2], outp);
                 outp += cells;
-                vz_step(M2(), zero, vzt[nvz - 1], outp);
+                vz_step(M2(), G1, G0, zero, vzt[nvz - 1], outp);
                 outp += cells;
             }
         }
