@@ -250,7 +250,11 @@ template <bool MOM> void *vstage_fn(int variant)
 #define MPHV_VS40_NS 3
 #endif
     case CUBE_40: return (void *)vstage_kernel<MPHV_VS40_NS, MOM, 40, 40, 416, 1>;
-    case CUBE_32: return (void *)vstage_kernel<2, MOM, 32, 32, 256, 2>;
+#ifndef MPHV_VS32_NS
+#define MPHV_VS32_NS 3          // measured on c2: ring depth 2 -> 3 and one 8-warp CTA per SM with up to 255 registers: 0.82 -> 0.67 ms
+#define MPHV_VS32_MINB 1
+#endif
+    case CUBE_32: return (void *)vstage_kernel<MPHV_VS32_NS, MOM, 32, 32, 256, MPHV_VS32_MINB>;
     case CUBE_36: return (void *)vstage_kernel<3, MOM, 36, 36, 352, 1>;
     case CUBE_16: return (void *)vstage_kernel<3, MOM, 16, 16, 64, 8>;
     default:      return (void *)vstage_kernel<3, MOM, 0, 0, 512, 1>;
@@ -260,13 +264,13 @@ template <bool MOM> void *vstage_bs_fn(int variant)
 {
     switch (variant) {
     case CUBE_40: return (void *)vstage_bs_kernel<MPHV_VS40_NS, MOM, 40, 40, 416, 1>;
-    case CUBE_32: return (void *)vstage_bs_kernel<2, MOM, 32, 32, 256, 2>;
+    case CUBE_32: return (void *)vstage_bs_kernel<MPHV_VS32_NS, MOM, 32, 32, 256, MPHV_VS32_MINB>;
     case CUBE_36: return (void *)vstage_bs_kernel<3, MOM, 36, 36, 352, 1>;
     case CUBE_16: return (void *)vstage_bs_kernel<3, MOM, 16, 16, 64, 8>;
     default:      return (void *)vstage_bs_kernel<3, MOM, 0, 0, 512, 1>;
     }
 }
-int vstage_ns(int variant) { return variant == CUBE_32 ? 2 : variant == CUBE_40 ? MPHV_VS40_NS : 3; }
+int vstage_ns(int variant) { return variant == CUBE_32 ? MPHV_VS32_NS : variant == CUBE_40 ? MPHV_VS40_NS : 3; }
 
 size_t vstage_smem_bytes(int nvx, int nvy, int nvz, int ns, int T)
 {
