@@ -82,7 +82,6 @@ vstage_kernel(const CubeArgs p)
         }
     }
 
-    const double dtdvx = p.dt / p.g.dv[0], dtdvy = p.dt / p.g.dv[1], dtdvz = p.dt / p.g.dv[2];
     // thread <-> work
     const int r_x = tid / qx, q_x = tid - r_x * qx;                       // V_vx item: row, quad
     const int rq = tid / nvx, jx = tid - rq * nvx;                        // V_vy / V_vz patch: row quad, column
@@ -92,9 +91,8 @@ vstage_kernel(const CubeArgs p)
     const int in_off = 4 * tid;                                          // doubles, within a ring plane
     const int xw_off = (r_x + 2) * nvx + 4 * q_x;                        // V_vx store, within an xb plane
     const int xr_off = r0 * nvx + jx;                                    // V_vy first row (r0 - 2, + 2 zero rows)
-    const double vy_row = vcentre(p.g, 1, act ? r_x : 0);                // V_vx: a_x needs vy of the row
-    const double vx_col = vcentre(p.g, 0, jx);                           // V_vy: a_y needs vx of the column
-    const double vy0 = vcentre(p.g, 1, act ? r0 : 0), dvy = p.g.dv[1];
+    // (per-thread velocity centres and dt / dv are re-evaluated in the peeled cube-boundary code, so they hold no
+    // registers across the iterations inside a cube)
 
     // per-cube linear forms of the Courant numbers: s = a + vz b
     double ax = 0.0, bx = 0.0, ay = 0.0, by = 0.0;
@@ -156,6 +154,7 @@ vstage_kernel(const CubeArgs p)
             if (AFIRST) {                            // new cube: a_x = qm (E_x + vy B_z - vz B_y)
                 const long long c = c_begin + cellA;
                 const double Ex = __ldg(p.E + c), By = __ldg(p.B + p.ns + c), Bz = __ldg(p.B + 2 * p.ns + c);
+                const double dtdvx = p.dt / p.g.dv[0], vy_row = vcentre(p.g, 1, act ? r_x : 0);   // a_x needs vy of the row
                 ax = (p.g.qm * (Ex + vy_row * Bz)) * dtdvx;
                 bx = -(p.g.qm * By) * dtdvx;
             }
@@ -203,6 +202,8 @@ vstage_kernel(const CubeArgs p)
             const double Ey = __ldg(p.E + p.ns + c), Ez = __ldg(p.E + 2 * p.ns + c);
             const double Bx = __ldg(p.B + c), By = __ldg(p.B + p.ns + c), Bz = __ldg(p.B + 2 * p.ns + c);
             // a_y = qm (E_y + vz B_x - vx B_z);  a_z = qm (E_z + vx B_y - vy B_x)
+            const double dtdvy = p.dt / p.g.dv[1], dtdvz = p.dt / p.g.dv[2], dvy = p.g.dv[1];
+            const double vx_col = vcentre(p.g, 0, jx), vy0 = vcentre(p.g, 1, act ? r0 : 0);
             ay = (p.g.qm * (Ey - vx_col * Bz)) * dtdvy;
             by = (p.g.qm * Bx) * dtdvy;
             const double az0 = Ez + vx_col * By;
@@ -275,6 +276,7 @@ vstage_kernel(const CubeArgs p)
                 for (int k = 0; k < 10; ++k) mom[k] = 0.0;
                 if (act) {
                     // sums over the thread's rows m = 0..3: vy = vy0 + m dvy
+                    const double dvy = p.g.dv[1], vx_col = vcentre(p.g, 0, jx), vy0 = vcentre(p.g, 1, r0);
                     const double Sy = fma(dvy, Q1, vy0 * P0);                                    // sum vy f
                     const double Syy = fma(dvy * dvy, Q2, fma(2.0 * vy0 * dvy, Q1, vy0 * vy0 * P0));
                     const double Syz = fma(dvy, ZQ, vy0 * Z1);
