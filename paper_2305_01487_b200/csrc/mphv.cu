@@ -6,6 +6,7 @@
 #include "mphv_vcube.cuh"
 #include "mphv_march.cuh"
 #include "mphv_vstage.cuh"
+#include "mphv_vstage2.cuh"
 #include "mphv_sxy.cuh"
 #include "mphv_backsub.cuh"
 #include "mphv_vstage_bs.cuh"
@@ -15,6 +16,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 #include <new>
 #include <vector>
 
@@ -24,6 +26,7 @@ struct mphv_ctx {
     mphv_grid grid;
     mphv_box box;
     double qm;
+    int dev;                 // CUDA device the context was created on (every entry point runs on it)
     cudaStream_t stream;
     double *f, *scratch;
     const double *E, *B;
@@ -36,7 +39,9 @@ struct mphv_ctx {
     int mom_tiles, mom_per_tile, mom_block;   // CTA tiling of the fused V_vz + moments kernel
     int sm_count;
     int vxy_T, vxy_grid; size_t vxy_smem;     // fused V_vx + V_vy plane kernel launch shape (0 = unsupported)
-    int vs_T, vs_grid, vs_variant, vs_bs; size_t vs_smem;   // second-generation whole-V-stage kernel (T = 0: unsupported)
+    int vs_T, vs_grid, vs_variant, vs_bs; size_t vs_smem;
+    int vs2_T, vs2_grid; size_t vs2_smem;            // third-generation whole-V-stage kernel, plain mode (T = 0: shape not covered)
+    unsigned char vs_afirst[16], vs_acnt[16];         // stage-A warp items per warp of vstage_kernel (balance_stage_a)   // second-generation whole-V-stage kernel (T = 0: unsupported)
     int sxy_T, sxy_C; size_t sxy_smem;               // fused S_x + S_y kernel (T = 0: unsupported)
     int cube_T, cube_grid, cube_variant, plane_grid; size_t cube_smem, plane_smem;  // whole-V-stage cube kernel launch shape (T = 0: unsupported)
     int vmode;                                       // 0 plain V sweeps, 1 backsubstitution
@@ -122,6 +127,17 @@ int after_launch(mphv_ctx *c, const char *what)
     if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(c, e, what); }
     return MPHV_OK;
 }
+
+// Makes the context's device current for the duration of one entry point and restores the caller's.
+struct DevGuard {
+    int prev; bool switched;
+    explicit DevGuard(const mphv_ctx *c) : prev(-1), switched(false)
+    {
+        if (!c) return;
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != c->dev) switched = cudaSetDevice(c->dev) == cudaSuccess;
+    }
+    ~DevGuard() { if (switched) cudaSetDevice(prev); }
+};
 
 bool is_finite(double x) { return x == x && !std::isinf(x); }
 
@@ -273,6 +289,29 @@ template <bool MOM> void *vstage_bs_fn(int variant)
     default:      return (void *)vstage_bs_kernel<3, MOM, 0, 0, 512, 1>;
     }
 }
+// third-generation whole-V-stage kernel (mphv_vstage2.cuh): velocity planes of the BASELINE.json configs and of
+// the paper's own grids. <ring depth, MOM, nvx, nvy, rows per patch, cells per run, threads, register-budget threads, CTAs per SM>
+#ifndef MPHV_VS2_NS40
+#define MPHV_VS2_NS40 3
+#endif
+template <bool MOM> void *vstage2_fn(int variant)
+{
+    switch (variant) {
+    case CUBE_40: return (void *)vstage2_kernel<MPHV_VS2_NS40, MOM, 40, 40, 5, 10, 320, 384, 1>;
+    case CUBE_32: return (void *)vstage2_kernel<3, MOM, 32, 32, 4, 8, 256, 256, 1>;
+    case CUBE_36: return (void *)vstage2_kernel<3, MOM, 36, 36, 6, 12, 224, 256, 1>;
+    case CUBE_16: return (void *)vstage2_kernel<3, MOM, 16, 16, 4, 8, 64, 64, 4>;
+    default:      return nullptr;
+    }
+}
+int vstage2_threads(int variant) { return variant == CUBE_40 ? 320 : variant == CUBE_32 ? 256 : variant == CUBE_36 ? 224 : variant == CUBE_16 ? 64 : 0; }
+int vstage2_ns(int variant) { return variant == CUBE_40 ? MPHV_VS2_NS40 : 3; }
+size_t vstage2_smem_bytes(int nvx, int nvy, int nvz, int ns)
+{
+    const size_t cells = (size_t)nvx * nvy, xcells = (size_t)nvx * (nvy + 4);
+    return (ns * 2 * cells + VS_NXB * 2 * xcells + nvz + 320) * sizeof(double) + (ns + 2) * sizeof(uint64_t);
+}
+
 int vstage_ns(int variant) { return variant == CUBE_32 ? MPHV_VS32_NS : variant == CUBE_40 ? MPHV_VS40_NS : 3; }
 
 size_t vstage_smem_bytes(int nvx, int nvy, int nvz, int ns, int T)
@@ -313,6 +352,7 @@ int launch_vcube(mphv_ctx *c, double dt, bool with_vz, double *n, double *j, dou
 // V_vx, V_vy, V_vz (+ moments if n != NULL) in one pass over f, two planes per pipeline iteration
 int launch_vstage(mphv_ctx *c, double dt, double *n, double *j, double *P, bool backsub = false)
 {
+    const bool gen3 = !backsub && c->vs2_T > 0;
     CubeArgs a;
     std::memset(&a, 0, sizeof a);
     a.f = c->f;
@@ -327,9 +367,11 @@ int launch_vstage(mphv_ctx *c, double dt, double *n, double *j, double *P, bool 
     Timed tm(c, n ? SLOT_VCUBE_MOM : SLOT_VCUBE, (n ? 56.0 : 48.0) * (double)c->nf);
     a.K = backsub ? c->bs_K : nullptr;
     void *fn = backsub ? (n ? vstage_bs_fn<true>(c->vs_variant) : vstage_bs_fn<false>(c->vs_variant))
+               : gen3  ? (n ? vstage2_fn<true>(c->vs_variant) : vstage2_fn<false>(c->vs_variant))
                        : (n ? vstage_fn<true>(c->vs_variant) : vstage_fn<false>(c->vs_variant));
     void *args[] = { &a };
-    cudaError_t e = cudaLaunchKernel(fn, dim3((unsigned)c->vs_grid), dim3((unsigned)c->vs_T), args, c->vs_smem, c->stream);
+    cudaError_t e = gen3 ? cudaLaunchKernel(fn, dim3((unsigned)c->vs2_grid), dim3((unsigned)c->vs2_T), args, c->vs2_smem, c->stream)
+                         : cudaLaunchKernel(fn, dim3((unsigned)c->vs_grid), dim3((unsigned)c->vs_T), args, c->vs_smem, c->stream);
     if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(c, e, "vstage_kernel launch"); }
     return after_launch(c, "vstage_kernel");
 }
@@ -620,6 +662,7 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
     std::memset(c, 0, sizeof *c);
     c->pending = new (std::nothrow) std::vector<mphv_ctx::Pending>();
     if (!c->pending) { set_err(nullptr, "out of host memory"); delete c; return nullptr; }
+    c->dev = dev;
     c->grid = *grid; c->box = *box; c->qm = q_over_m;
     c->ns = (size_t)grid->nx[0] * grid->nx[1] * grid->nx[2];
     c->nvel = (size_t)grid->nv[0] * grid->nv[1] * grid->nv[2];
@@ -715,6 +758,21 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
                        cudaFuncSetAttribute(vstage_bs_fn<false>(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess;
         }
         cudaGetLastError();
+        c->vs2_T = 0;
+        if (c->vs_T > 0 && vstage2_fn<true>(variant)) {
+            const size_t smem2 = vstage2_smem_bytes(nvx, nvy, nvz, vstage2_ns(variant));
+            const int T2 = vstage2_threads(variant);
+            int per2 = 0;
+            if (smem2 <= (size_t)max_optin &&
+                cudaFuncSetAttribute(vstage2_fn<true>(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2) == cudaSuccess &&
+                cudaFuncSetAttribute(vstage2_fn<false>(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2) == cudaSuccess &&
+                cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per2, vstage2_fn<true>(variant), T2, smem2) == cudaSuccess && per2 > 0) {
+                long long g2 = (long long)per2 * c->sm_count;
+                if (g2 > (long long)c->ns) g2 = (long long)c->ns;
+                c->vs2_T = T2; c->vs2_smem = smem2; c->vs2_grid = (int)g2;
+            }
+            cudaGetLastError();
+        }
     }
     c->sxy_T = 0;
     if (grid->nx[0] >= 8 && grid->nx[0] % 4 == 0 && grid->nx[1] >= 4) {
@@ -749,6 +807,7 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
 
 int mphv_destroy(mphv_ctx *c)
 {
+    DevGuard dg(c);
     if (!c) return MPHV_ERR_ARG;
     if (c->ws) cudaFree(c->ws);
     if (c->fld) cudaFree(c->fld);
@@ -760,6 +819,7 @@ int mphv_destroy(mphv_ctx *c)
 
 int mphv_set_stream(mphv_ctx *c, void *s)
 {
+    DevGuard dg(c);
     if (!c) return MPHV_ERR_ARG;
     c->stream = (cudaStream_t)s;
     return MPHV_OK;
@@ -770,6 +830,7 @@ size_t mphv_space_count(const mphv_ctx *c) { return c ? c->ns : 0; }
 
 int mphv_bind_f(mphv_ctx *c, double *f, double *scratch)
 {
+    DevGuard dg(c);
     if (!c) return MPHV_ERR_ARG;
     if (!f) { set_err(c, "f_dev is NULL"); return MPHV_ERR_ARG; }
     if (((uintptr_t)f & 15) || ((uintptr_t)scratch & 15)) { set_err(c, "f/scratch must be 16-byte aligned"); return MPHV_ERR_ARG; }
@@ -780,6 +841,7 @@ int mphv_bind_f(mphv_ctx *c, double *f, double *scratch)
 
 int mphv_set_fields(mphv_ctx *c, const double *E, const double *B)
 {
+    DevGuard dg(c);
     if (!c) return MPHV_ERR_ARG;
     if (!E || !B) { set_err(c, "E_dev or B_dev is NULL"); return MPHV_ERR_ARG; }
     double *out = ws_scalars(c);
@@ -801,6 +863,7 @@ int mphv_set_fields(mphv_ctx *c, const double *E, const double *B)
 
 int mphv_sweep_x(mphv_ctx *c, int dim, double dt)
 {
+    DevGuard dg(c);
     int st = check_common(c, dt, false);
     if (st != MPHV_OK) return st;
     if (dim < 0 || dim > 2 || c->grid.nx[dim] < 2) { set_err(c, "spatial dim %d out of range or inactive", dim); return MPHV_ERR_ARG; }
@@ -811,6 +874,7 @@ int mphv_sweep_x(mphv_ctx *c, int dim, double dt)
 
 int mphv_sweep_v(mphv_ctx *c, int dim, double dt)
 {
+    DevGuard dg(c);
     int st = check_common(c, dt, true);
     if (st != MPHV_OK) return st;
     if (dim < 0 || dim > 2 || c->grid.nv[dim] < 2) { set_err(c, "velocity dim %d out of range or inactive", dim); return MPHV_ERR_ARG; }
@@ -851,10 +915,15 @@ static int step_impl(mphv_ctx *c, double dt, double *n, double *j, double *P)
     return do_v_stage(c, dt, n, j, P);
 }
 
-int mphv_step(mphv_ctx *c, double dt) { return step_impl(c, dt, nullptr, nullptr, nullptr); }
+int mphv_step(mphv_ctx *c, double dt)
+{
+    DevGuard dg(c);
+    return step_impl(c, dt, nullptr, nullptr, nullptr);
+}
 
 int mphv_moments(mphv_ctx *c, double *n, double *j, double *P)
 {
+    DevGuard dg(c);
     if (!c) return MPHV_ERR_ARG;
     if (!n || !j || !P) { set_err(c, "n_dev, j_dev or P_dev is NULL"); return MPHV_ERR_ARG; }
     if (!c->f) { set_err(c, "f not bound (mphv_bind_f)"); return MPHV_ERR_STATE; }
@@ -863,6 +932,7 @@ int mphv_moments(mphv_ctx *c, double *n, double *j, double *P)
 
 int mphv_stage_x(mphv_ctx *c, double dt)
 {
+    DevGuard dg(c);
     int st = check_common(c, dt, false);
     if (st != MPHV_OK) return st;
     for (int d = 0; d < 3; ++d)
@@ -872,6 +942,7 @@ int mphv_stage_x(mphv_ctx *c, double dt)
 
 int mphv_stage_v(mphv_ctx *c, double dt, double *n, double *j, double *P)
 {
+    DevGuard dg(c);
     int st = check_common(c, dt, true);
     if (st != MPHV_OK) return st;
     if (n && (!j || !P)) { set_err(c, "n_dev given but j_dev or P_dev is NULL"); return MPHV_ERR_ARG; }
@@ -888,6 +959,7 @@ size_t mphv_halo_count(const mphv_ctx *c, int dim)
 
 int mphv_pack_halo(mphv_ctx *c, int dim, int side, double *buf)
 {
+    DevGuard dg(c);
     if (!c) return MPHV_ERR_ARG;
     if (dim < 0 || dim > 2 || c->grid.nx[dim] < 2) { set_err(c, "spatial dim %d out of range or inactive", dim); return MPHV_ERR_ARG; }
     if (side != 0 && side != 1) { set_err(c, "side must be 0 (low end) or 1 (high end)"); return MPHV_ERR_ARG; }
@@ -905,6 +977,7 @@ int mphv_pack_halo(mphv_ctx *c, int dim, int side, double *buf)
 
 int mphv_sweep_x_halo(mphv_ctx *c, int dim, double dt, const double *lo, const double *hi)
 {
+    DevGuard dg(c);
     int st = check_common(c, dt, false);
     if (st != MPHV_OK) return st;
     if (dim < 0 || dim > 2 || c->grid.nx[dim] < 2) { set_err(c, "spatial dim %d out of range or inactive", dim); return MPHV_ERR_ARG; }
@@ -921,6 +994,7 @@ int mphv_sweep_x_halo(mphv_ctx *c, int dim, double dt, const double *lo, const d
 
 int mphv_maxwellian(mphv_ctx *c, size_t count, const double *n, const double *j, const double *P, double *f_out)
 {
+    DevGuard dg(c);
     if (!c) return MPHV_ERR_ARG;
     if (!n || !j || !P || !f_out) { set_err(c, "n_dev, j_dev, P_dev or f_out_dev is NULL"); return MPHV_ERR_ARG; }
     if (count == 0) return MPHV_OK;
@@ -934,6 +1008,7 @@ int mphv_maxwellian(mphv_ctx *c, size_t count, const double *n, const double *j,
 
 int mphv_exchange_maxwellian(mphv_ctx *c, int dim, int side, const double *n_fl, const double *j_fl, const double *P_fl)
 {
+    DevGuard dg(c);
     if (!c) return MPHV_ERR_ARG;
     if (dim < 0 || dim > 2 || c->grid.nx[dim] < 4) { set_err(c, "spatial dim %d out of range or inactive", dim); return MPHV_ERR_ARG; }
     if (side != 0 && side != 1) { set_err(c, "side must be 0 (low end) or 1 (high end)"); return MPHV_ERR_ARG; }
@@ -954,6 +1029,7 @@ int mphv_exchange_maxwellian(mphv_ctx *c, int dim, int side, const double *n_fl,
 
 int mphv_match_moments(mphv_ctx *c, const double *n_t, const double *j_t, const double *P_t)
 {
+    DevGuard dg(c);
     if (!c) return MPHV_ERR_ARG;
     if (!n_t || !j_t || !P_t) { set_err(c, "n_t_dev, j_t_dev or P_t_dev is NULL"); return MPHV_ERR_ARG; }
     if (!c->f) { set_err(c, "f not bound (mphv_bind_f)"); return MPHV_ERR_STATE; }
@@ -967,6 +1043,7 @@ int mphv_match_moments(mphv_ctx *c, const double *n_t, const double *j_t, const 
 
 int mphv_stage_x_halo(mphv_ctx *c, double dt, const double *lo, const double *hi)
 {
+    DevGuard dg(c);
     int st = check_common(c, dt, false);
     if (st != MPHV_OK) return st;
     if (c->grid.nx[0] < 2) { set_err(c, "spatial dim 0 is inactive"); return MPHV_ERR_ARG; }
@@ -996,6 +1073,7 @@ int mphv_stage_x_halo(mphv_ctx *c, double dt, const double *lo, const double *hi
 
 int mphv_step_moments(mphv_ctx *c, double dt, double *n, double *j, double *P)
 {
+    DevGuard dg(c);
     if (!c) return MPHV_ERR_ARG;
     if (!n || !j || !P) { set_err(c, "n_dev, j_dev or P_dev is NULL"); return MPHV_ERR_ARG; }
     return step_impl(c, dt, n, j, P);
@@ -1003,6 +1081,7 @@ int mphv_step_moments(mphv_ctx *c, double dt, double *n, double *j, double *P)
 
 int mphv_run_host(mphv_ctx *c, double *f_host, int nsteps, double dt, double *n_host, double *j_host, double *P_host)
 {
+    DevGuard dg(c);
     int st = step_checks(c, dt);
     if (st != MPHV_OK) return st;
     if (!f_host || nsteps < 0) { set_err(c, "f_host is NULL or nsteps < 0"); return MPHV_ERR_ARG; }
@@ -1024,6 +1103,7 @@ int mphv_run_host(mphv_ctx *c, double *f_host, int nsteps, double dt, double *n_
 int mphv_step_fields_host(mphv_ctx *c, const double *E_host, const double *B_host, double dt,
                           double *n_host, double *j_host, double *P_host)
 {
+    DevGuard dg(c);
     if (!c) return MPHV_ERR_ARG;
     if (!E_host || !B_host || !n_host || !j_host || !P_host) { set_err(c, "a host pointer is NULL"); return MPHV_ERR_ARG; }
     if (!c->f) { set_err(c, "f not bound (mphv_bind_f)"); return MPHV_ERR_STATE; }
@@ -1046,6 +1126,7 @@ int mphv_step_fields_host(mphv_ctx *c, const double *E_host, const double *B_hos
 
 int mphv_sum_f(mphv_ctx *c, double *sum_dev)
 {
+    DevGuard dg(c);
     if (!c) return MPHV_ERR_ARG;
     if (!sum_dev) { set_err(c, "sum_dev is NULL"); return MPHV_ERR_ARG; }
     if (!c->f) { set_err(c, "f not bound (mphv_bind_f)"); return MPHV_ERR_STATE; }
@@ -1060,6 +1141,7 @@ int mphv_sum_f(mphv_ctx *c, double *sum_dev)
 
 int mphv_set_timing(mphv_ctx *c, int enabled)
 {
+    DevGuard dg(c);
     if (!c) return MPHV_ERR_ARG;
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     drain_timing(c, false);
@@ -1073,6 +1155,7 @@ int mphv_timing_slots(void) { return SLOT_COUNT; }
 int mphv_get_timing(mphv_ctx *c, int slot, char *name, size_t name_cap, double *total_ms,
                     uint64_t *launches, double *alg_bytes_per_launch)
 {
+    DevGuard dg(c);
     if (!c) return MPHV_ERR_ARG;
     if (slot < 0 || slot >= SLOT_COUNT) { set_err(c, "timing slot %d out of range", slot); return MPHV_ERR_ARG; }
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
@@ -1088,6 +1171,7 @@ uint64_t mphv_launch_count(const mphv_ctx *c) { return c ? c->launches : 0; }
 
 int mphv_set_vmode(mphv_ctx *c, int mode)
 {
+    DevGuard dg(c);
     if (!c) return MPHV_ERR_ARG;
     if (mode != MPHV_V_PLAIN && mode != MPHV_V_BACKSUB) { set_err(c, "vmode must be MPHV_V_PLAIN or MPHV_V_BACKSUB"); return MPHV_ERR_ARG; }
     if (mode == MPHV_V_BACKSUB) {
@@ -1106,6 +1190,7 @@ int mphv_set_vmode(mphv_ctx *c, int mode)
 
 int mphv_set_fusion(mphv_ctx *c, int enabled)
 {
+    DevGuard dg(c);
     if (!c) return MPHV_ERR_ARG;
     c->fusion = enabled < 0 ? 0 : (enabled > 3 ? 3 : enabled);
     return MPHV_OK;

@@ -286,6 +286,12 @@ class Vlasov:
             raise ValueError(f"need a contiguous float64 tensor of {count} elements on {self.device}")
         return t.data_ptr()
 
+    def _host(self, t, count):
+        torch = self.torch
+        if t.dtype != torch.float64 or not t.is_contiguous() or t.numel() != count or t.device.type != "cpu":
+            raise ValueError(f"need a contiguous float64 CPU tensor of {count} elements")
+        return t.data_ptr()
+
     def close(self):
         if self.ctx:
             mphv_destroy(self.ctx)
@@ -323,29 +329,35 @@ class Vlasov:
                 torch.empty((3,) + sp, dtype=torch.float64, device=self.device),
                 torch.empty((6,) + sp, dtype=torch.float64, device=self.device))
 
+    def _mom_ptrs(self, n, j, P):
+        """Device pointers of a moment triple after the dtype / contiguity / size / device check."""
+        ns = mphv_space_count(self.ctx)
+        return self._dev(n, ns), self._dev(j, 3 * ns), self._dev(P, 6 * ns)
+
     def moments(self, out=None):
         n, j, P = out if out is not None else self.alloc_moments()
-        mphv_moments(self.ctx, n.data_ptr(), j.data_ptr(), P.data_ptr())
+        mphv_moments(self.ctx, *self._mom_ptrs(n, j, P))
         return n, j, P
 
     def step_moments(self, dt, out=None):
         n, j, P = out if out is not None else self.alloc_moments()
-        mphv_step_moments(self.ctx, dt, n.data_ptr(), j.data_ptr(), P.data_ptr())
+        mphv_step_moments(self.ctx, dt, *self._mom_ptrs(n, j, P))
         return n, j, P
 
     def stage_x(self, dt):
         mphv_stage_x(self.ctx, dt)
 
     def stage_x_halo(self, dt, lo=None, hi=None):
-        mphv_stage_x_halo(self.ctx, dt, None if lo is None else lo.data_ptr(), None if hi is None else hi.data_ptr())
+        cnt = self.halo_count(0)
+        mphv_stage_x_halo(self.ctx, dt, None if lo is None else self._dev(lo, cnt),
+                          None if hi is None else self._dev(hi, cnt))
 
     def stage_v(self, dt, out=None):
         """The V stage alone; with out = (n, j, P) tensors the moments of the result are written too."""
         if out is None:
             mphv_stage_v(self.ctx, dt)
             return None
-        n, j, P = out
-        mphv_stage_v(self.ctx, dt, n.data_ptr(), j.data_ptr(), P.data_ptr())
+        mphv_stage_v(self.ctx, dt, *self._mom_ptrs(*out))
         return out
 
     def halo_count(self, dim) -> int:
@@ -368,14 +380,17 @@ class Vlasov:
 
     def run_host(self, f_host, nsteps, dt, n_host=None, j_host=None, P_host=None):
         """f_host etc.: CPU float64 tensors (pinned for speed); updated in place."""
-        def hp(t):
-            return None if t is None else t.data_ptr()
-        mphv_run_host(self.ctx, f_host.data_ptr(), nsteps, dt, hp(n_host), hp(j_host), hp(P_host))
+        ns = mphv_space_count(self.ctx)
+        mphv_run_host(self.ctx, self._host(f_host, mphv_f_count(self.ctx)), nsteps, dt,
+                      None if n_host is None else self._host(n_host, ns),
+                      None if j_host is None else self._host(j_host, 3 * ns),
+                      None if P_host is None else self._host(P_host, 6 * ns))
 
     def step_fields_host(self, E_host, B_host, dt, n_host, j_host, P_host):
         """Coupled step with f resident: host fields in, host moments out (CPU float64 tensors, pinned for speed)."""
-        mphv_step_fields_host(self.ctx, E_host.data_ptr(), B_host.data_ptr(), dt,
-                              n_host.data_ptr(), j_host.data_ptr(), P_host.data_ptr())
+        ns = mphv_space_count(self.ctx)
+        mphv_step_fields_host(self.ctx, self._host(E_host, 3 * ns), self._host(B_host, 3 * ns), dt,
+                              self._host(n_host, ns), self._host(j_host, 3 * ns), self._host(P_host, 6 * ns))
 
     @property
     def launches(self) -> int:
@@ -383,18 +398,22 @@ class Vlasov:
 
     def maxwellian(self, n, j, P, out=None):
         """Ten-moment Maxwellian cubes of n.numel() cells (device tensors n [count], j [3][count], P [6][count])."""
-        import torch
+        torch = self.torch
         count = n.numel()
+        nvel = self.nv[0] * self.nv[1] * self.nv[2]
         if out is None:
-            out = torch.empty((count, self.nv[2], self.nv[1], self.nv[0]), dtype=torch.float64, device=n.device)
-        mphv_maxwellian(self.ctx, count, n.data_ptr(), j.data_ptr(), P.data_ptr(), out.data_ptr())
+            out = torch.empty((count, self.nv[2], self.nv[1], self.nv[0]), dtype=torch.float64, device=self.device)
+        mphv_maxwellian(self.ctx, count, self._dev(n, count), self._dev(j, 3 * count), self._dev(P, 6 * count),
+                        self._dev(out, count * nvel))
         return out
 
     def match_moments(self, n_t, j_t, P_t):
-        mphv_match_moments(self.ctx, n_t.data_ptr(), j_t.data_ptr(), P_t.data_ptr())
+        mphv_match_moments(self.ctx, *self._mom_ptrs(n_t, j_t, P_t))
 
     def exchange_maxwellian(self, dim, side, n_fl, j_fl, P_fl):
-        mphv_exchange_maxwellian(self.ctx, dim, side, n_fl.data_ptr(), j_fl.data_ptr(), P_fl.data_ptr())
+        """n_fl [2][plane], j_fl [3][2][plane], P_fl [6][2][plane]: fluid moments of the two boundary layers."""
+        cnt = 2 * (mphv_space_count(self.ctx) // self.nx[dim])
+        mphv_exchange_maxwellian(self.ctx, dim, side, self._dev(n_fl, cnt), self._dev(j_fl, 3 * cnt), self._dev(P_fl, 6 * cnt))
 
     def set_vmode(self, mode):
         mphv_set_vmode(self.ctx, mode)

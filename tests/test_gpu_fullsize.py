@@ -93,3 +93,54 @@ def test_full_size_step_moments_on_sampled_cells(orc, index):
         for a_g, a_r in [(n_g[None], n_r[None]), (j_g, j_r), (P_g, P_r)]:
             d = np.abs(a_g[:, cell[2], cell[1], cell[0]] - a_r[:, c[2], c[1], c[0]])
             assert np.max(d) <= 1e-12 * sc, f"{w.name} cell {cell}: moments"
+
+
+def _rel_err_by_slab(f_gpu, ref, slab_axis=1):
+    """parity_util.rel_err (5-point neighbourhood along vz, the last-swept axis) of the whole grid, one spatial
+    slab at a time so that the host never holds more than one extra slab of temporaries."""
+    worst = 0.0
+    for i in range(ref.shape[slab_axis]):
+        sl = [slice(None)] * ref.ndim
+        sl[slab_axis] = slice(i, i + 1)
+        r = ref[tuple(sl)]
+        g = f_gpu[tuple(sl)].cpu().numpy()
+        scale = np.maximum(local_scale(r, 3), 1e-300)
+        worst = max(worst, float(np.max(np.abs(g - r) / scale)))
+    return worst
+
+
+@pytest.mark.parametrize("index", [2, 3])
+def test_whole_grid_all_steps_of_the_config(orc, index):
+    """BASELINE.json configs 2 and 3 as they are written: the config's 10 full split steps on the WHOLE grid, every
+    cell compared with the oracle (1e-12 after the first step, n x 1e-12 after n), mass to 1e-13 every step,
+    moments every step (config 2) or after the last one (config 3), in the launch configuration bench.py times."""
+    import torch
+    from paper_2305_01487_b200 import inputs, mphv
+    w = inputs.config(index)
+    f0, E, B, dt = inputs.make_all(w)
+    grid, box = orc.Grid(w.nx, w.nv, w.bc), orc.Box(w.xlo, w.xhi, w.vlo, w.vhi)
+    sim = mphv.Vlasov.from_workload(w)
+    f = torch.from_numpy(f0).cuda()
+    sim.bind_f(f)
+    sim.set_fields(torch.from_numpy(E).cuda(), torch.from_numpy(B).cuda())
+    mom = sim.alloc_moments()
+    ref = f0
+    del f0
+    every = index == 2
+    for s in range(w.steps):
+        orc.step(ref, grid, box, w.q_over_m, E, B, dt)
+        if every or s == w.steps - 1:
+            sim.step_moments(dt, mom)
+        else:
+            sim.step(dt)
+        m_ref = orc.total(ref)
+        assert abs(sim.sum_f() - m_ref) <= 1e-13 * abs(m_ref), f"{w.name} step {s + 1}: mass"
+        if every or s == w.steps - 1:
+            n_r, j_r, P_r = orc.moments(ref, grid, box)
+            sc = np.abs(P_r[0]) + np.abs(P_r[3]) + np.abs(P_r[5]) + np.abs(n_r)
+            for a_g, a_r in zip(mom, (n_r, j_r, P_r)):
+                assert np.max(np.abs(a_g.cpu().numpy() - a_r) / sc) <= (s + 1) * 1e-12, f"{w.name} step {s + 1}: moments"
+        if s == 0:
+            assert _rel_err_by_slab(f, ref) <= TOL_SWEEP, f"{w.name}: a single step must meet 1e-12 in every cell"
+    assert float(f.min()) >= 0.0
+    assert _rel_err_by_slab(f, ref) <= w.steps * TOL_SWEEP, f"{w.name}: {w.steps} steps, every cell"

@@ -4,7 +4,7 @@ V-stage mode; two steps + moments against the oracle, element by element."""
 import numpy as np
 import pytest
 
-from parity_util import local_scale
+from parity_util import local_scale, rel_err
 from test_gpu_parity import torch_cuda, mphv  # noqa: F401
 
 pytestmark = pytest.mark.gpu
@@ -46,11 +46,17 @@ def test_random_configurations_match_the_oracle(torch_cuda, mphv, orc, seed):
             n, j, P = sim.step_moments(dt)
         torch.cuda.synchronize()
         got = f.cpu().numpy()
-        scale = np.abs(ref)
-        for ax in (3, 4, 5):
-            scale = local_scale(scale, ax)
         tag = f"nx {nx} nv {nv} bc {bc} fusion {fusion} vmode {vmode}"
-        assert np.max(np.abs(got - ref) / np.maximum(scale, 1e-300)) <= 2e-12, tag
+        if vmode == 0:
+            # plain sweeps: the metric of SURVEY 8(c) -- 5-point neighbourhood along the last-swept axis (vz)
+            assert rel_err(got, ref, axis=3) <= 2e-12, tag
+        else:
+            # backsubstitution: each of the three face-displaced sweeps leaves an error proportional to its own
+            # stencil (the displacement varies along the pencil), so the neighbourhood spans all three axes
+            scale = np.abs(ref)
+            for ax in (3, 4, 5):
+                scale = local_scale(scale, ax)
+            assert np.max(np.abs(got - ref) / np.maximum(scale, 1e-300)) <= 2e-12, tag
         n_r, j_r, P_r = orc.moments(ref, grid, box)
         sc = np.abs(P_r[0]) + np.abs(P_r[3]) + np.abs(P_r[5]) + np.abs(n_r)
         for a, b in [(n, n_r), (j, j_r), (P, P_r)]:
