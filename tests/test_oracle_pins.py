@@ -569,3 +569,14 @@ def test_step_is_x_y_then_vx_vy_vz_and_budget(orc):
     for _ in range(10):
         assert orc.step(c, gridp, box, w.q_over_m, E, B, dt) == 0.0
     assert abs(orc.total(c) - m0) <= 1e-13 * m0
+
+
+def test_total_is_the_exactly_rounded_sum(orc):
+    """orc.total against math.fsum (the exactly rounded sum) on data that defeats a plain running sum: one large
+    entry followed by many entries below half an ulp of it, and a Maxwellian-like spread over 60 decades."""
+    from math import fsum
+    a = np.concatenate([[1.0e5], np.full(1_000_000, 1.0e-16), [-1.0e5], np.full(1000, 3.0e-17)])
+    assert abs(orc.total(a) - fsum(a)) <= 1e-18 * fsum(np.abs(a))      # a plain long double sum returns 0 here
+    rng = np.random.default_rng(7)
+    b = np.exp(-rng.uniform(0.0, 140.0, 400_000))
+    assert abs(orc.total(b) - fsum(b)) <= 1e-16 * fsum(b)
