@@ -198,6 +198,95 @@ def run_reference(args, w):
     print(json.dumps(line), flush=True)
 
 
+
+# ------------------------------------------------------------------------------- roofline
+# What limits each kernel (profiles/r02_*_ncu_full.md): the whole-V-stage kernels are bound by instruction
+# issue / latency (their DRAM rate is about half the copy rate at 100 % of the bytes they must move), every
+# other kernel by HBM.
+KERNEL_BOUND = {"fused_vx_vy_vz_moments": "issue", "fused_vx_vy_vz": "issue", "match_moments": "issue"}
+COUNTERS = ROOT / "profiles" / "kernel_counters.json"
+
+
+def csrc_sha16() -> str:
+    """Hash of the CUDA sources: ncu counters in profiles/kernel_counters.json are only quoted while it matches."""
+    import hashlib
+    h = hashlib.sha256()
+    for p in sorted((ROOT / "paper_2305_01487_b200" / "csrc").glob("*.cu*")):
+        h.update(p.name.encode()); h.update(p.read_bytes())
+    return h.hexdigest()[:16]
+
+
+def sim_sm_count(torch, index: int) -> int:
+    return int(torch.cuda.get_device_properties(index).multi_processor_count)
+
+
+def make_roofline(timings, steps, ms_per_step, peak_gbs, peak_src, clocks, sm_count, w):
+    """The roofline object of the bench line. For the dominant kernel (largest share of the step):
+    achieved = bytes the launch MUST move (f read once + written once per pass, whatever it fuses) / its mean
+    CUDA-event duration; frac = achieved / measured copy rate -- a physical fraction, <= ~1. The survey's
+    contract currency (algorithmic bytes of the UNFUSED sweeps) is kept under *_algorithmic_unfused: fusion makes
+    it exceed 1. traffic = DRAM bytes ncu measured for that kernel, quoted only while the sources are unchanged."""
+    kern = {k: dict(v, ms_per_launch=v["ms"] / v["launches"]) for k, v in timings.items()}
+    dom = max(kern, key=lambda k: kern[k]["ms"])
+    d = kern[dom]
+    total_ms = sum(v["ms"] for v in kern.values())
+    step_alg = sum(v["alg_bytes"] * v["launches"] for v in kern.values()) / steps
+    step_moved = sum(v["moved_bytes"] * v["launches"] for v in kern.values()) / steps
+    achieved = d["moved_bytes"] / (d["ms_per_launch"] * 1e-3) / 1e9
+    counters, note = {}, None
+    try:
+        cj = json.loads(COUNTERS.read_text())
+        if cj.get("csrc_sha16") == csrc_sha16() and cj.get("workload") == w.name:
+            counters = cj.get("kernels", {})
+        else:
+            note = (f"profiles/kernel_counters.json was measured at commit {cj.get('commit')} on {cj.get('workload')}; "
+                    "the CUDA sources or the workload differ now, so no ncu counter is quoted")
+    except Exception as e:  # noqa: BLE001
+        note = f"no profiles/kernel_counters.json ({e!r})"
+    cd = counters.get(dom, {})
+    sm_hz = 1e6 * float(clocks.get("sm_mhz") or clocks.get("sm_max_mhz") or 1965.0)
+    issue_peak = sm_count * 4 * sm_hz                     # one warp instruction per scheduler per cycle
+    r = {
+        "bound": KERNEL_BOUND.get(dom, "hbm"), "kernel": dom,
+        "achieved": achieved, "peak": peak_gbs, "unit": "GB/s", "frac": achieved / peak_gbs,
+        "what": "bytes the dominant kernel must move per launch (one read + one write of f) / its CUDA-event time, "
+                "against the measured copy rate",
+        "peak_source": f"{peak_src} (MEASURED_PEAKS.json hbm_gbs)" if peak_src == "measured" else "fallback 6650 GB/s",
+        "traffic": cd.get("dram_bytes"),
+        "share_of_step": d["ms"] / total_ms,
+        "frac_algorithmic_unfused": d["alg_bytes"] / (d["ms_per_launch"] * 1e-3) / 1e9 / peak_gbs,
+        "step": {"moved_GBps": step_moved / (ms_per_step * 1e-3) / 1e9,
+                 "frac": step_moved / (ms_per_step * 1e-3) / 1e9 / peak_gbs,
+                 "algorithmic_unfused_GBps": step_alg / (ms_per_step * 1e-3) / 1e9,
+                 "frac_algorithmic_unfused_of_8TBps": step_alg / (ms_per_step * 1e-3) / 8e12,
+                 "frac_algorithmic_unfused_of_measured": step_alg / (ms_per_step * 1e-3) / 1e9 / peak_gbs},
+        "kernels": {},
+    }
+    if note:
+        r["traffic_note"] = note
+    elif counters:
+        r["traffic_source"] = f"profiles/kernel_counters.json (ncu --set full, commit {cj.get('commit')})"
+    for k, v in kern.items():
+        e = {"bound": KERNEL_BOUND.get(k, "hbm"), "ms_per_launch": round(v["ms_per_launch"], 4),
+             "launches_per_step": v["launches"] / steps,
+             "moved_GBps": round(v["moved_bytes"] / (v["ms_per_launch"] * 1e-3) / 1e9, 1),
+             "frac": round(v["moved_bytes"] / (v["ms_per_launch"] * 1e-3) / 1e9 / peak_gbs, 4),
+             "algorithmic_unfused_GBps": round(v["alg_bytes"] / (v["ms_per_launch"] * 1e-3) / 1e9, 1)}
+        ck = counters.get(k, {})
+        if ck.get("warp_instructions"):
+            # issue roofline: executed warp instructions (ncu smsp__inst_executed.sum) / time against one
+            # instruction per scheduler per cycle at the SM clock seen during the run
+            rate = ck["warp_instructions"] / (v["ms_per_launch"] * 1e-3)
+            e["issue"] = {"warp_instructions": ck["warp_instructions"],
+                          "thread_instructions_per_cell": round(32.0 * ck["warp_instructions"] / w.n_cells, 2),
+                          "achieved_Ginstr_s": round(rate / 1e9, 1), "peak_Ginstr_s": round(issue_peak / 1e9, 1),
+                          "frac": round(rate / issue_peak, 4)}
+        r["kernels"][k] = e
+    if "issue" in r["kernels"][dom]:
+        r["issue"] = r["kernels"][dom]["issue"]
+    return r
+
+
 # ------------------------------------------------------------------------------- CUDA arm
 def run_mphv(args, w):
     import torch
@@ -262,16 +351,18 @@ def run_mphv(args, w):
         step_moments(dt, mom)
     barrier()
     launches0 = sim.launches
-    sim.set_timing(True)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sim.set_timing(True)          # per-launch CUDA events inside the timed region (conservative: they cost a little)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     with ClockSampler(local) as clk:
         barrier()
-        e0.record()
-        for _ in range(args.steps):
+        ev[0].record()
+        for k in range(args.steps):
             step_moments(dt, mom)
-        e1.record()
+            ev[k + 1].record()
         barrier()
-    ms = e0.elapsed_time(e1)
+    e0, e1 = ev[0], ev[-1]
+    ms = e0.elapsed_time(e1)                                      # EXACTLY args.steps steps, one bracket
+    per_step = sorted(ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps))   # the same steps, one by one
     launches = sim.launches - launches0
     timings = sim.timings()
     sim.set_timing(False)
@@ -285,30 +376,8 @@ def run_mphv(args, w):
     # sanity of the timed state: f finite, non-negative, moments finite
     assert bool(torch.isfinite(mom[0]).all()) and float(f.min()) >= 0.0
 
-    # dominant kernel and its roofline (algorithmic bytes / CUDA-event duration)
-    kern = {k: dict(v, ms_per_launch=v["ms"] / v["launches"]) for k, v in timings.items()}
-    dom = max(kern, key=lambda k: kern[k]["ms"])
-    d = kern[dom]
-    achieved = d["alg_bytes"] / (d["ms_per_launch"] * 1e-3) / 1e9
-    step_alg_bytes = sum(v["alg_bytes"] * v["launches"] for v in kern.values()) / args.steps
-    roofline = {
-        "bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak_gbs, "unit": "GB/s",
-        "frac": achieved / peak_gbs, "peak_source": f"{peak_src} (MEASURED_PEAKS.json hbm_gbs)" if peak_src == "measured" else "fallback 6650 GB/s",
-        "traffic": None,
-        "share_of_step": d["ms"] / sum(v["ms"] for v in kern.values()),
-        "step_algorithmic_GBps": step_alg_bytes / (ms_per_step * 1e-3) / 1e9,
-        "step_frac_of_8TBps": step_alg_bytes / (ms_per_step * 1e-3) / 8e12,
-        "step_frac_of_measured": step_alg_bytes / (ms_per_step * 1e-3) / 1e9 / peak_gbs,
-        "kernels": {k: {"ms_per_launch": round(v["ms_per_launch"], 4), "launches_per_step": v["launches"] / args.steps,
-                        "alg_GBps": round(v["alg_bytes"] / (v["ms_per_launch"] * 1e-3) / 1e9, 1)} for k, v in kern.items()},
-    }
-    tr = ROOT / "profiles" / "traffic.json"
-    if tr.exists():
-        try:
-            roofline["traffic"] = json.loads(tr.read_text()).get(dom)
-        except Exception:  # noqa: BLE001
-            pass
-
+    clocks = clk.summary()
+    roofline = make_roofline(timings, args.steps, ms_per_step, peak_gbs, peak_src, clocks, sim_sm_count(torch, local), w)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(3, args.warmup), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
@@ -320,7 +389,10 @@ def run_mphv(args, w):
                    "parallelism": "1 GPU" if world == 1 else
                    (f"{world} spatial blocks along periodic x, 2-layer halo exchange before S_x (NCCL send/recv), "
                     f"{2 * sim.halo_count(0) * 8} B sent per rank per step" if halo_mode else f"{world} independent problems")},
-        "clocks": clk.summary(), "gpu_launches": launches, "roofline": roofline,
+        "clocks": clocks, "gpu_launches": launches, "roofline": roofline,
+        "ms_per_step_median": per_step[len(per_step) // 2], "ms_per_step_min": per_step[0], "ms_per_step_max": per_step[-1],
+        "timing": f"one CUDA-event bracket around the {args.steps} steps (value, ms_per_step); median/min/max over the same "
+                  f"{args.steps} steps timed one by one; per-launch CUDA events are recorded inside the timed region",
     }
 
     # end to end through the C ABI with HOST buffers: H2D(f) + step + moments + D2H(f, moments) per step

@@ -189,6 +189,10 @@ int mphv_set_timing(mphv_ctx *ctx, int enabled);
 int mphv_timing_slots(void);
 int mphv_get_timing(mphv_ctx *ctx, int slot, char *name, size_t name_cap, double *total_ms,
                     uint64_t *launches, double *alg_bytes_per_launch);
+/* The bytes ONE launch of slot `slot` has to move through HBM whatever it fuses: f read once and written
+ * once per PASS over f (16 B/cell for a fused stage of several sweeps, 8 for a moments pass). This is the
+ * numerator of the physical HBM roofline fraction; the algorithmic figure above counts every fused sweep. */
+int mphv_get_timing_moved(mphv_ctx *ctx, int slot, double *moved_bytes_per_launch);
 
 /* ---- model coupling at a Vlasov / ten-moment border (sec. 4.3; readings R16, R17).
  * mphv_maxwellian: f_out_dev[c][nvel] = the ten-moment Maxwellian ("a multivariate normal distribution",

@@ -10,3 +10,4 @@ from .binding import (  # noqa: F401
     maxwellian, exchange_maxwellian, match_moments,
     BC_PERIODIC, BC_OUTFLOW, BC_WALL, OK, ERR_ARG, ERR_RANGE,
 )
+from . import fields  # noqa: F401,E402  (FDTD Maxwell update and the coupled step)

@@ -15,6 +15,7 @@ import numpy as np
 
 _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "mphv_oracle.c"
+_SRCS = [_SRC, _HERE / "mphv_fields_oracle.c"]
 _SO = _HERE / "libmphv_oracle.so"
 
 BC_PERIODIC, BC_OUTFLOW, BC_WALL = 0, 1, 2
@@ -62,7 +63,7 @@ class Box:
 
 def build(force: bool = False) -> Path:
     """Compile the oracle: -O2, OpenMP over independent pencils, no FMA contraction."""
-    if not force and _SO.exists() and _SO.stat().st_mtime >= _SRC.stat().st_mtime:
+    if not force and _SO.exists() and all(_SO.stat().st_mtime >= p.stat().st_mtime for p in _SRCS):
         return _SO
     cands = [c for c in ("/usr/bin/gcc", shutil.which("gcc"), shutil.which("cc")) if c]
     flags = ["-O2", "-std=c99", "-ffp-contract=off", "-fPIC", "-shared", "-Wall", "-Wextra"]
@@ -70,7 +71,7 @@ def build(force: bool = False) -> Path:
     for cc in cands:
         for omp in (["-fopenmp"], []):
             tmp = _SO.with_suffix(f".{os.getpid()}.tmp")
-            r = subprocess.run([cc, *flags, *omp, "-o", str(tmp), str(_SRC), "-lm"],
+            r = subprocess.run([cc, *flags, *omp, "-o", str(tmp), *map(str, _SRCS), "-lm"],
                                capture_output=True, text=True)
             if r.returncode == 0:
                 os.replace(tmp, _SO)

@@ -55,6 +55,7 @@ struct mphv_ctx {
     double slot_ms[24];
     uint64_t slot_launches[24];
     double slot_bytes[24];
+    double slot_moved[24];
     char err[512];
 };
 
@@ -90,12 +91,14 @@ int cuda_fail(mphv_ctx *c, cudaError_t e, const char *what)
 // Brackets one kernel launch with CUDA events when timing is on.
 struct Timed {
     mphv_ctx *c; int slot; cudaEvent_t e0, e1; bool on;
-    Timed(mphv_ctx *c_, int slot_, double alg_bytes) : c(c_), slot(slot_), e0(nullptr), e1(nullptr), on(false)
+    // alg_bytes: algorithmic (unfused) bytes of the launch; moved_bytes: what ONE pass must move (< 0: the same)
+    Timed(mphv_ctx *c_, int slot_, double alg_bytes, double moved_bytes = -1.0) : c(c_), slot(slot_), e0(nullptr), e1(nullptr), on(false)
     {
         if (!c->timing) return;
         if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) { cudaGetLastError(); return; }
         on = true;
         c->slot_bytes[slot] = alg_bytes;
+        c->slot_moved[slot] = moved_bytes < 0.0 ? alg_bytes : moved_bytes;
         cudaEventRecord(e0, c->stream);
     }
     ~Timed()
@@ -200,7 +203,7 @@ double *ws_scalars(mphv_ctx *c) { return ws_sum(c) + SUM_BLOCKS; }
 // V_vz with the moments of the new f accumulated in the same kernel (f read once less)
 int launch_vz_moments(mphv_ctx *c, MarchArgs a, double *n, double *j, double *P)
 {
-    Timed tm(c, SLOT_VZMOM, 24.0 * (double)c->nf);
+    Timed tm(c, SLOT_VZMOM, 24.0 * (double)c->nf, 16.0 * (double)c->nf);
     a.mom = ws_partials(c);
     a.tiles = c->mom_tiles;
     a.per_tile = c->mom_per_tile;
@@ -226,7 +229,7 @@ int launch_vxy(mphv_ctx *c, double dt)
     a.dt = dt;
     a.E = c->E; a.B = c->B;
     a.g = c->gd;
-    Timed tm(c, SLOT_VXY, 32.0 * (double)c->nf);
+    Timed tm(c, SLOT_VXY, 32.0 * (double)c->nf, 16.0 * (double)c->nf);
     const long long grid = a.planes < c->vxy_grid ? a.planes : c->vxy_grid;
     vxy_kernel<3><<<(unsigned)grid, c->vxy_T, c->vxy_smem, c->stream>>>(a);
     return after_launch(c, "vxy_kernel");
@@ -340,7 +343,7 @@ int launch_vcube(mphv_ctx *c, double dt, bool with_vz, double *n, double *j, dou
     a.n = n; a.j = j; a.P = P;
     a.dV = c->dv[0] * c->dv[1] * c->dv[2];
     a.g = c->gd;
-    Timed tm(c, !with_vz ? SLOT_VXY : n ? SLOT_VCUBE_MOM : SLOT_VCUBE, (!with_vz ? 32.0 : n ? 56.0 : 48.0) * (double)c->nf);
+    Timed tm(c, !with_vz ? SLOT_VXY : n ? SLOT_VCUBE_MOM : SLOT_VCUBE, (!with_vz ? 32.0 : n ? 56.0 : 48.0) * (double)c->nf, 16.0 * (double)c->nf);
     void *fn = !with_vz ? plane_fn(c->cube_variant) : n ? cube_fn<true>(c->cube_variant) : cube_fn<false>(c->cube_variant);
     void *args[] = { &a };
     cudaError_t e = cudaLaunchKernel(fn, dim3((unsigned)(with_vz ? c->cube_grid : c->plane_grid)), dim3((unsigned)c->cube_T), args,
@@ -364,7 +367,7 @@ int launch_vstage(mphv_ctx *c, double dt, double *n, double *j, double *P, bool 
     a.dV = c->dv[0] * c->dv[1] * c->dv[2];
     a.sixth = 1.0 / 6.0;
     a.g = c->gd;
-    Timed tm(c, n ? SLOT_VCUBE_MOM : SLOT_VCUBE, (n ? 56.0 : 48.0) * (double)c->nf);
+    Timed tm(c, n ? SLOT_VCUBE_MOM : SLOT_VCUBE, (n ? 56.0 : 48.0) * (double)c->nf, 16.0 * (double)c->nf);
     a.K = backsub ? c->bs_K : nullptr;
     void *fn = backsub ? (n ? vstage_bs_fn<true>(c->vs_variant) : vstage_bs_fn<false>(c->vs_variant))
                : gen3  ? (n ? vstage2_fn<true>(c->vs_variant) : vstage2_fn<false>(c->vs_variant))
@@ -410,7 +413,7 @@ int launch_sxy(mphv_ctx *c, double dt, bool halo = false, const double *lo = nul
     a.chunks = (int)(c->nvel / (size_t)c->sxy_C);
     a.dt = dt; a.dx = c->dx[0]; a.dy = c->dx[1];
     a.g = c->gd;
-    Timed tm(c, SLOT_SXY, 32.0 * (double)c->nf);
+    Timed tm(c, SLOT_SXY, 32.0 * (double)c->nf, 16.0 * (double)c->nf);
     a.halo_lo = lo; a.halo_hi = hi;
     void *fn = sxy_fn(c->sxy_C, halo ? SXY_BCX_HALO : c->grid.bc[0], c->grid.bc[1]);
     void *args[] = { &a };
@@ -1145,7 +1148,7 @@ int mphv_set_timing(mphv_ctx *c, int enabled)
     if (!c) return MPHV_ERR_ARG;
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     drain_timing(c, false);
-    for (int i = 0; i < 24; ++i) { c->slot_ms[i] = 0.0; c->slot_launches[i] = 0; c->slot_bytes[i] = 0.0; }
+    for (int i = 0; i < 24; ++i) { c->slot_ms[i] = 0.0; c->slot_launches[i] = 0; c->slot_bytes[i] = 0.0; c->slot_moved[i] = 0.0; }
     c->timing = enabled ? 1 : 0;
     return MPHV_OK;
 }
@@ -1164,6 +1167,14 @@ int mphv_get_timing(mphv_ctx *c, int slot, char *name, size_t name_cap, double *
     if (total_ms) *total_ms = c->slot_ms[slot];
     if (launches) *launches = c->slot_launches[slot];
     if (alg_bytes_per_launch) *alg_bytes_per_launch = c->slot_bytes[slot];
+    return MPHV_OK;
+}
+
+int mphv_get_timing_moved(mphv_ctx *c, int slot, double *moved_bytes_per_launch)
+{
+    if (!c) return MPHV_ERR_ARG;
+    if (slot < 0 || slot >= SLOT_COUNT || !moved_bytes_per_launch) { set_err(c, "timing slot %d out of range or NULL output", slot); return MPHV_ERR_ARG; }
+    *moved_bytes_per_launch = c->slot_moved[slot];
     return MPHV_OK;
 }
 

@@ -26,7 +26,7 @@ SYMBOLS = (
     "mphv_bind_f", "mphv_set_fields", "mphv_sweep_x", "mphv_sweep_v", "mphv_step",
     "mphv_moments", "mphv_step_moments", "mphv_run_host", "mphv_step_fields_host", "mphv_sum_f", "mphv_launch_count",
     "mphv_set_fusion", "mphv_set_vmode", "mphv_maxwellian", "mphv_exchange_maxwellian", "mphv_match_moments", "mphv_strerror", "mphv_last_error",
-    "mphv_set_timing", "mphv_timing_slots", "mphv_get_timing",
+    "mphv_set_timing", "mphv_timing_slots", "mphv_get_timing", "mphv_get_timing_moved",
     "mphv_stage_x", "mphv_stage_x_halo", "mphv_stage_v", "mphv_halo_count", "mphv_pack_halo", "mphv_sweep_x_halo",
 )
 
@@ -84,6 +84,7 @@ def lib() -> C.CDLL:
         "mphv_timing_slots": (i32, []),
         "mphv_get_timing": (i32, [vp, i32, C.c_char_p, C.c_size_t, C.POINTER(dbl),
                                   C.POINTER(C.c_uint64), C.POINTER(dbl)]),
+        "mphv_get_timing_moved": (i32, [vp, i32, C.POINTER(dbl)]),
         "mphv_stage_x": (i32, [vp, dbl]),
         "mphv_stage_x_halo": (i32, [vp, dbl, vp, vp]),
         "mphv_stage_v": (i32, [vp, dbl, vp, vp, vp]),
@@ -255,6 +256,13 @@ def mphv_get_timing(ctx, slot: int):
     ms, n, b = C.c_double(0.0), C.c_uint64(0), C.c_double(0.0)
     _check(ctx, lib().mphv_get_timing(ctx, int(slot), name, 64, C.byref(ms), C.byref(n), C.byref(b)))
     return name.value.decode(), ms.value, int(n.value), b.value
+
+
+def mphv_get_timing_moved(ctx, slot: int) -> float:
+    """Bytes one launch of the slot must move through HBM (one read + one write of f per pass)."""
+    b = C.c_double(0.0)
+    _check(ctx, lib().mphv_get_timing_moved(ctx, int(slot), C.byref(b)))
+    return b.value
 
 
 # ------------------------------------------------------------------ torch convenience
@@ -430,5 +438,5 @@ class Vlasov:
         for s in range(mphv_timing_slots()):
             name, ms, n, b = mphv_get_timing(self.ctx, s)
             if n:
-                out[name] = dict(ms=ms, launches=n, alg_bytes=b)
+                out[name] = dict(ms=ms, launches=n, alg_bytes=b, moved_bytes=mphv_get_timing_moved(self.ctx, s))
         return out
