@@ -119,6 +119,8 @@ def lib() -> C.CDLL:
         L.orc_exchange_maxwellian.restype = C.c_int
         L.orc_match_moments.argtypes = [dp, C.POINTER(_CGrid), C.POINTER(_CBox), dp, dp, dp]
         L.orc_match_moments.restype = C.c_int
+        L.orc_set_num_threads.argtypes = [C.c_int]
+        L.orc_set_num_threads.restype = None
         L.orc_num_threads.argtypes = []
         L.orc_num_threads.restype = C.c_int
         _lib = L
@@ -289,3 +291,8 @@ def total(f: np.ndarray) -> float:
 
 def num_threads() -> int:
     return int(lib().orc_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    """OpenMP threads of later oracle calls (tiny grids run much faster on one thread)."""
+    lib().orc_set_num_threads(int(n))

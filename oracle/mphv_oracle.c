@@ -824,6 +824,16 @@ double orc_sum(const double *f, size_t count)
     return (double)(acc + comp);
 }
 
+/* Number of OpenMP threads later calls use (small grids run faster on one). No-op without OpenMP. */
+void orc_set_num_threads(int n)
+{
+#ifdef _OPENMP
+    if (n >= 1) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
 int orc_num_threads(void)
 {
     int nt = 1;
