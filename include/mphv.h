@@ -246,6 +246,87 @@ int mphv_set_vmode(mphv_ctx *ctx, int mode);
  * Results agree up to fp64 rounding at every level. */
 int mphv_set_fusion(mphv_ctx *ctx, int level);
 
+/* mphv_set_fields without the host round trip, for coupled runs that change the fields every step (P:L109,
+ * P:L141): the max |a_d| reduction is enqueued as in mphv_set_fields but its result stays on the device, and the
+ * MPHV_ERR_RANGE check of every later velocity sweep / V stage / step is made ON THE DEVICE when that call is
+ * enqueued (one 1-thread kernel in front of it) and raises a sticky device flag instead of failing the call.
+ * mphv_deferred_status synchronises the stream and returns MPHV_ERR_RANGE if the flag was raised since the last
+ * query (and clears it), else MPHV_OK. A sweep enqueued with |s| >= 1 computes a wrong remap of f (no out-of-bounds
+ * access): after MPHV_ERR_RANGE from mphv_deferred_status f must be considered lost. mphv_set_fields switches back
+ * to the immediate check. E_dev, B_dev are borrowed as in mphv_set_fields; if they are changed in place, one of the
+ * two set_fields calls MUST be made again before the next velocity sweep. */
+int mphv_set_fields_deferred(mphv_ctx *ctx, const double *E_dev, const double *B_dev);
+int mphv_deferred_status(mphv_ctx *ctx);
+
+/* ---- closing the loop: Maxwell's equations fed by the species' currents, and the coupled step.
+ * eq. (9): curl E = -dB/dt, curl B = mu0 j + mu0 eps0 dE/dt, j = sum_s q_s n_s u_s; "solved via the finite
+ * difference time domain (FDTD) method", div B = 0 by construction; "The Maxwell solver itself uses Strang
+ * splitting between E and B". Readings R19..R22 of DESIGN.md:
+ *   R19  Yee lattice on the Vlasov cells, integer indices = cell centres: array element [k][j][i] of
+ *        Ex at (i+1/2, j, k), Ey at (i, j+1/2, k), Ez at (i, j, k+1/2)   (faces normal to the component),
+ *        Bx at (i, j+1/2, k+1/2), By at (i+1/2, j, k+1/2), Bz at (i+1/2, j+1/2, k)   (edges along the component);
+ *        no derivative and no staggering along an inactive axis.
+ *   R20  E_d at a centre = mean of its 2 faces along d; B_d at a centre = mean of its 4 edges in the plane normal
+ *        to d; the current on the face of E_d = mean of the two adjacent cell-centred values.
+ *   R21  periodic axis = index wrap, bounded axis (MPHV_BC_OUTFLOW) = zero-gradient ghost value.
+ * All field arrays: device, [3][nz][ny][nx], component-major, owned by the caller. Calls only enqueue. */
+typedef struct mphv_maxwell mphv_maxwell;
+
+typedef struct {
+    int32_t nx[3];                     /* spatial extents (as mphv_grid.nx)                                */
+    int32_t bc[3];                     /* MPHV_BC_PERIODIC or MPHV_BC_OUTFLOW (zero-gradient ghosts, R21)   */
+    double dx[3];                      /* cell widths; ignored along inactive axes                          */
+    double c2;                         /* c^2 = 1 / (mu0 eps0)                                              */
+    double inv_eps0;                   /* 1 / eps0                                                          */
+} mphv_field_grid;
+
+mphv_maxwell *mphv_maxwell_create(const mphv_field_grid *grid);     /* NULL on error: mphv_last_error(NULL)  */
+int mphv_maxwell_destroy(mphv_maxwell *m);
+int mphv_maxwell_set_stream(mphv_maxwell *m, void *cuda_stream);
+/* The staggered fields (R19) the later calls update in place. */
+int mphv_maxwell_bind(mphv_maxwell *m, double *E_dev, double *B_dev);
+/* B <- B - dt curl E (Faraday). */
+int mphv_maxwell_faraday(mphv_maxwell *m, double dt);
+/* E <- E + dt (c^2 curl B - J / eps0) (Ampere-Maxwell); J_dev = cell-centred charge current or NULL (vacuum). */
+int mphv_maxwell_ampere(mphv_maxwell *m, const double *J_dev, double dt);
+/* One Maxwell step with J frozen: B(dt/2), E(dt; J), B(dt/2). One launch on grids up to 65536 cells. */
+int mphv_maxwell_step(mphv_maxwell *m, const double *J_dev, double dt);
+/* Fields at the cell centres (R20): what mphv_set_fields takes (R8). */
+int mphv_maxwell_centre(mphv_maxwell *m, double *Ec_dev, double *Bc_dev);
+/* Charge current J = sum_s q_s j_s (eq. (9)); q_host[nspecies], j_dev_ptrs = HOST array of nspecies device
+ * pointers to the species' number fluxes j = int v f d3v ([3][ns] each, as mphv_moments writes them); nspecies <= 4. */
+int mphv_maxwell_current(mphv_maxwell *m, int nspecies, const double *q_host, const double *const *j_dev_ptrs,
+                         double *J_dev);
+const char *mphv_maxwell_last_error(const mphv_maxwell *m);
+
+/* A set of kinetic species coupled through Maxwell's equations: the paper's Scheme {Vlasov e, Vlasov i, Maxwell}
+ * (P:L109). The species contexts (each with f bound, created on the same device with the spatial grid of
+ * the field solver) and the field solver (fields bound) belong to the caller and must outlive the plasma object;
+ * q_host[s] is the charge that weights species s in the current (its q/m lives in its context).
+ * mphv_plasma_step: nsteps steps of the coupled scheme R22 (leapfrog-like Strang between plasma and fields, P:L135,
+ * P:L145), per step
+ *        J = sum_s q_s j_s[f_s];  Maxwell(dt/2; J);  E_c, B_c = centred fields;
+ *        every species: f_s <- mphv_step(dt) with E_c, B_c frozen, moments of the new f_s;
+ *        J' = sum_s q_s j_s[f_s];  Maxwell(dt/2; J').
+ * Every species runs on a CUDA stream of its own (concurrent = 1) so that one species' HBM-bound spatial sweeps can
+ * overlap another's issue-bound V stage, the field update on a third; they are ordered by events, the host never
+ * waits inside the loop (velocity RANGE checks are deferred, see mphv_set_fields_deferred). concurrent = 0 runs
+ * everything on one stream (for comparison). The call returns after the last step has been enqueued and the streams
+ * have been joined on the field solver's stream; mphv_plasma_sync waits for it and reports a deferred RANGE error.
+ * The first call computes the moments of the initial f_s itself.
+ * mphv_plasma_moments: device pointers to the latest moments of species s (n [ns], j [3][ns], P [6][ns], owned by
+ * the plasma object, valid after mphv_plasma_sync). */
+typedef struct mphv_plasma mphv_plasma;
+mphv_plasma *mphv_plasma_create(mphv_maxwell *m, int nspecies, mphv_ctx *const *species, const double *q_host);
+int mphv_plasma_destroy(mphv_plasma *p);
+int mphv_plasma_set_concurrent(mphv_plasma *p, int concurrent);
+int mphv_plasma_step(mphv_plasma *p, double dt, int nsteps);
+int mphv_plasma_sync(mphv_plasma *p);
+int mphv_plasma_moments(mphv_plasma *p, int s, double **n_dev, double **j_dev, double **P_dev);
+/* centred fields of the last step (device, [3][ns] each, owned by the plasma object) */
+int mphv_plasma_centred_fields(mphv_plasma *p, double **Ec_dev, double **Bc_dev);
+const char *mphv_plasma_last_error(const mphv_plasma *p);
+
 const char *mphv_strerror(int code);
 /* Last error text of this context, or of the last failed mphv_create when ctx is NULL.
  * The returned pointer is owned by the library and valid until the next failing call. */

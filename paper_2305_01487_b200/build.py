@@ -15,14 +15,15 @@ PKG = Path(__file__).resolve().parent
 ROOT = PKG.parent
 CSRC = PKG / "csrc"
 SO = PKG / "libmphv.so"
-SOURCES = [CSRC / "mphv.cu"]
+SOURCES = [CSRC / "mphv.cu", CSRC / "mphv_coupled.cu"]
 DEPS = SOURCES + sorted(CSRC.glob("*.cuh")) + [ROOT / "include" / "mphv.h"]
 
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-lineinfo",
     "-gencode", "arch=compute_100a,code=sm_100a",
-    "-Xcompiler", "-fPIC", "-shared", "-cudart", "static",
+    "-Xcompiler", "-fPIC",
 ]
+LINK_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-cudart", "static"]
 
 
 def nvcc() -> str:
@@ -40,17 +41,25 @@ def build(force: bool = False, verbose: bool = False, extra: list[str] | None = 
     if not force and up_to_date():
         return SO
     tmp = SO.with_suffix(f".{os.getpid()}.tmp")
-    cmd = [nvcc(), *NVCC_FLAGS, *(extra or []), "-I", str(ROOT / "include"),
-           "-o", str(tmp), *map(str, SOURCES)]
-    if verbose:
-        cmd.insert(1, "-Xptxas")
-        cmd.insert(2, "-v")
-    r = subprocess.run(cmd, capture_output=True, text=True)
-    if verbose:
-        sys.stderr.write(r.stderr)
-    if r.returncode != 0:
-        tmp.unlink(missing_ok=True)
-        raise RuntimeError("nvcc failed:\n" + " ".join(cmd) + "\n" + r.stdout + r.stderr)
+    objs = [PKG / f".{src.stem}.{os.getpid()}.o" for src in SOURCES]
+    cmds = [[nvcc(), *NVCC_FLAGS, *(extra or []), *(["-Xptxas", "-v"] if verbose else []),
+             "-I", str(ROOT / "include"), "-c", "-o", str(o), str(src)] for src, o in zip(SOURCES, objs)]
+    procs = [subprocess.Popen(c, stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True) for c in cmds]   # in parallel
+    outs = [p.communicate() for p in procs]
+    try:
+        for c, p, (so, se) in zip(cmds, procs, outs):
+            if verbose:
+                sys.stderr.write(se)
+            if p.returncode != 0:
+                raise RuntimeError("nvcc failed:\n" + " ".join(c) + "\n" + so + se)
+        link = [nvcc(), *LINK_FLAGS, "-o", str(tmp), *map(str, objs)]
+        r = subprocess.run(link, capture_output=True, text=True)
+        if r.returncode != 0:
+            tmp.unlink(missing_ok=True)
+            raise RuntimeError("nvcc link failed:\n" + " ".join(link) + "\n" + r.stdout + r.stderr)
+    finally:
+        for o in objs:
+            o.unlink(missing_ok=True)
     os.replace(tmp, SO)
     return SO
 

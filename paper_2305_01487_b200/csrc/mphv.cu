@@ -34,6 +34,7 @@ struct mphv_ctx {
     double dx[3], dv[3];
     GridDev gd;
     double amax[3];          // max |a_d| over all pencils, from the last set_fields
+    bool deferred;           // mphv_set_fields_deferred: the bounds stay on the device, RANGE checks raise a device flag
     double *fld;             // device copy of host fields for mphv_step_fields_host: [3 ns] E | [3 ns] B (lazy)
     double *ws;              // device workspace: [10 ns] moments | [10 ns mom_tiles] partials | [SUM_BLOCKS] | [8]
     int mom_tiles, mom_per_tile, mom_block;   // CTA tiling of the fused V_vz + moments kernel
@@ -489,8 +490,10 @@ int ensure_backsub(mphv_ctx *c, double dt)
         st = after_launch(c, "backsub_coeff_kernel");
     }
     if (st != MPHV_OK) return st;
-    CUDA_TRY(c, cudaMemcpyAsync(c->bs_smax, smax, 3 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
-    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    if (!c->deferred) {
+        CUDA_TRY(c, cudaMemcpyAsync(c->bs_smax, smax, 3 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    }
     c->bs_dt = dt; c->bs_valid = true;
     return MPHV_OK;
 }
@@ -551,12 +554,14 @@ int do_sweep_v(mphv_ctx *c, int d, double dt)
 }
 
 int do_moments(mphv_ctx *c, double *n, double *j, double *P);
+int enqueue_range_flag(mphv_ctx *c, double dt);
 
 // The whole V stage (active velocity sweeps in order vx, vy, vz) and, if n != NULL, the moments
 // of the result. With fusion on: [vx+vy in one plane kernel], [vz + moments in one kernel].
 int do_v_stage(mphv_ctx *c, double dt, double *n, double *j, double *P)
 {
     int st;
+    if (c->deferred && (st = enqueue_range_flag(c, dt)) != MPHV_OK) return st;
     const bool ax = c->grid.nv[0] > 1, ay = c->grid.nv[1] > 1, az = c->grid.nv[2] > 1;
     if (c->vmode && c->fusion >= 2 && c->vs_T > 0 && c->vs_bs) return launch_vstage(c, dt, n, j, P, true);
     if (c->vmode) {                                  // backsubstitution: three face-displaced sweeps, then the moments
@@ -615,8 +620,23 @@ int range_x(mphv_ctx *c, int d, double dt)
     return MPHV_OK;
 }
 
+// deferred mode: one 1-thread kernel compares the device-resident bounds of all active velocity axes with 1
+// and raises the sticky flag ws_scalars[4]
+int enqueue_range_flag(mphv_ctx *c, double dt)
+{
+    int active = 0;
+    for (int d = 0; d < 3; ++d) if (c->grid.nv[d] > 1) active |= 1 << d;
+    const double *bound = c->vmode ? c->bs_K + 12 * c->ns : ws_scalars(c);
+    range_flag_kernel<<<1, 32, 0, c->stream>>>(bound, dt, c->dv[0], c->dv[1], c->dv[2], active, c->vmode ? 0 : 1, ws_scalars(c) + 4);
+    return after_launch(c, "range_flag_kernel");
+}
+
 int range_v(mphv_ctx *c, int d, double dt)
 {
+    if (c->deferred) {
+        if (c->vmode) return ensure_backsub(c, dt);
+        return MPHV_OK;                              // checked on the device (enqueue_range_flag)
+    }
     if (c->vmode) {
         int st = ensure_backsub(c, dt);
         if (st != MPHV_OK) return st;
@@ -626,7 +646,8 @@ int range_v(mphv_ctx *c, int d, double dt)
         }
         return MPHV_OK;
     }
-    const double smax = max_courant_v(c, d, dt);
+    // the fused kernels form s as fma(v, b, a) with dt / dv folded in: up to a few ulp away from (a dt) / dv
+    const double smax = max_courant_v(c, d, dt) * (1.0 + 1.0e-15);
     if (!(smax < 1.0)) { set_err(c, "velocity sweep %d: max |s| = %g >= 1 (closed velocity box)", d, smax); return MPHV_ERR_RANGE; }
     return MPHV_OK;
 }
@@ -634,6 +655,9 @@ int range_v(mphv_ctx *c, int d, double dt)
 }  // namespace
 
 extern "C" {
+
+// for the other translation unit of the library (mphv_coupled.cu): text of mphv_last_error(NULL)
+void mphv_internal_set_create_error(const char *text) { set_err(nullptr, "%s", text ? text : ""); }
 
 mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_m)
 {
@@ -842,6 +866,42 @@ int mphv_bind_f(mphv_ctx *c, double *f, double *scratch)
     return MPHV_OK;
 }
 
+int mphv_set_fields_deferred(mphv_ctx *c, const double *E, const double *B)
+{
+    DevGuard dg(c);
+    if (!c) return MPHV_ERR_ARG;
+    if (!E || !B) { set_err(c, "E_dev or B_dev is NULL"); return MPHV_ERR_ARG; }
+    int st;
+    {
+        Timed tm(c, SLOT_AMAX, 0.0);
+        amax_kernel<<<1, 1024, 0, c->stream>>>(E, B, c->gd, ws_scalars(c));
+        st = after_launch(c, "amax_kernel");
+    }
+    if (st != MPHV_OK) return st;
+    if (!c->deferred) CUDA_TRY(c, cudaMemsetAsync(ws_scalars(c) + 4, 0, sizeof(double), c->stream));
+    c->E = E; c->B = B;
+    c->bs_valid = false;
+    c->deferred = true;
+    for (int d = 0; d < 3; ++d) c->amax[d] = NAN;
+    return MPHV_OK;
+}
+
+int mphv_deferred_status(mphv_ctx *c)
+{
+    DevGuard dg(c);
+    if (!c) return MPHV_ERR_ARG;
+    if (!c->deferred) return MPHV_OK;
+    double flag = 0.0;
+    CUDA_TRY(c, cudaMemcpyAsync(&flag, ws_scalars(c) + 4, sizeof flag, cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    if (flag != 0.0) {
+        CUDA_TRY(c, cudaMemsetAsync(ws_scalars(c) + 4, 0, sizeof(double), c->stream));
+        set_err(c, "a velocity sweep enqueued since the last query had |s| >= 1 (deferred RANGE check): f is lost");
+        return MPHV_ERR_RANGE;
+    }
+    return MPHV_OK;
+}
+
 int mphv_set_fields(mphv_ctx *c, const double *E, const double *B)
 {
     DevGuard dg(c);
@@ -855,6 +915,7 @@ int mphv_set_fields(mphv_ctx *c, const double *E, const double *B)
         st = after_launch(c, "amax_kernel");
     }
     if (st != MPHV_OK) return st;
+    c->deferred = false;
     double h[3];
     CUDA_TRY(c, cudaMemcpyAsync(h, out, sizeof h, cudaMemcpyDeviceToHost, c->stream));
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
@@ -883,6 +944,7 @@ int mphv_sweep_v(mphv_ctx *c, int dim, double dt)
     if (dim < 0 || dim > 2 || c->grid.nv[dim] < 2) { set_err(c, "velocity dim %d out of range or inactive", dim); return MPHV_ERR_ARG; }
     st = range_v(c, dim, dt);
     if (st != MPHV_OK) return st;
+    if (c->deferred && (st = enqueue_range_flag(c, dt)) != MPHV_OK) return st;
     return do_sweep_v(c, dim, dt);
 }
 

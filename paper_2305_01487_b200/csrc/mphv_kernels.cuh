@@ -623,4 +623,20 @@ amax_kernel(const double *__restrict__ E, const double *__restrict__ B, GridDev 
     }
 }
 
+// deferred RANGE check of the velocity sweeps (no host round trip): bound[d] = max |a_d| (plain mode, scaled here
+// by dt / dv_d as the host check does) or max |s_face| (backsubstitution, scale 1); *flag becomes 1 and stays 1
+// when a bound is not below 1.
+__global__ void range_flag_kernel(const double *bound, double dt, double dv0, double dv1, double dv2, int active, int scaled, double *flag)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    const double dv[3] = { dv0, dv1, dv2 };
+    bool bad = false;
+    for (int d = 0; d < 3; ++d) {
+        if (!((active >> d) & 1)) continue;
+        const double s = scaled ? fabs(__ddiv_rn(__dmul_rn(bound[d], dt), dv[d])) : bound[d];
+        if (!(s * (1.0 + 1.0e-15) < 1.0)) bad = true;
+    }
+    if (bad) *flag = 1.0;
+}
+
 }  // namespace mphv

@@ -47,6 +47,8 @@ class Workload:
     background: float = 0.2         # n_b of the Harris sheets
     guide_bz: float = 0.0
     seed_offset: int = 0            # extra offset for test variants
+    sigma: float = 1.0              # thermal spread (standard deviation) of the Maxwellians
+    drift: float = 0.5              # |u_z| of the current-carrying sheet population
 
     @property
     def shape(self):
@@ -215,8 +217,10 @@ def cfl_dt(w: Workload, E: np.ndarray, B: np.ndarray) -> float:
 
 # --------------------------------------------------------------------------- f0
 
-def _gauss(v: np.ndarray, u: float = 0.0) -> np.ndarray:
-    return np.exp(-0.5 * (v - u) ** 2) / np.sqrt(2.0 * np.pi)
+def _gauss(v: np.ndarray, u: float = 0.0, sigma: float = 1.0) -> np.ndarray:
+    if sigma == 1.0:
+        return np.exp(-0.5 * (v - u) ** 2) / np.sqrt(2.0 * np.pi)
+    return np.exp(-0.5 * ((v - u) / sigma) ** 2) / (np.sqrt(2.0 * np.pi) * sigma)
 
 
 def make_f0(w: Workload, noise: float = 1e-6, density_ripple: float = 1e-3) -> np.ndarray:
@@ -240,17 +244,18 @@ def make_f0(w: Workload, noise: float = 1e-6, density_ripple: float = 1e-3) -> n
         return np.ascontiguousarray(f.reshape(w.shape))
 
     y = w.x_centres(1)
-    gx, gy = _gauss(w.v_centres(0)), _gauss(w.v_centres(1))
+    sg = w.sigma
+    gx, gy = _gauss(w.v_centres(0), 0.0, sg), _gauss(w.v_centres(1), 0.0, sg)
     vz = w.v_centres(2)
     ripple = 1.0 + density_ripple * _smooth_noise(w, rng)            # (nz, ny, nx)
     if w.kind == "harris2d":
-        sheets = [(1.0 / np.cosh(y / 0.5) ** 2, 0.5)]
+        sheets = [(1.0 / np.cosh(y / 0.5) ** 2, w.drift)]
     else:
-        sheets = [(1.0 / np.cosh((y + 3.2) / 0.5) ** 2, 0.5),
-                  (1.0 / np.cosh((y - 3.2) / 0.5) ** 2, -0.5)]
+        sheets = [(1.0 / np.cosh((y + 3.2) / 0.5) ** 2, w.drift),
+                  (1.0 / np.cosh((y - 3.2) / 0.5) ** 2, -w.drift)]
     # z-profile in velocity per spatial row: sum_sheets n_s(y) G(vz - u_s) + n_b G(vz)
-    zprof = w.background * _gauss(vz)[None, :] + sum(
-        n_s[:, None] * _gauss(vz, u)[None, :] for n_s, u in sheets)  # (ny, nvz)
+    zprof = w.background * _gauss(vz, 0.0, sg)[None, :] + sum(
+        n_s[:, None] * _gauss(vz, u, sg)[None, :] for n_s, u in sheets)  # (ny, nvz)
     plane = gy[:, None] * gx[None, :]                                # (nvy, nvx)
     f = np.empty(w.shape)
     for iz in range(nz):
@@ -271,3 +276,36 @@ def make_all(w: Workload):
 
 def variant(w: Workload, **kw) -> Workload:
     return replace(w, **kw)
+
+
+def electrons_of(w: Workload, mass_ratio: float = 100.0, temp_ratio: float = 0.2, nv: int = 36,
+                 vmax: float = 20.0) -> Workload:
+    """The electron species that goes with the (ion) Harris workload w in a two-species run: same spatial
+    grid and density profile (a neutral plasma), q/m = -mass_ratio, velocity grid nv^3 on [-vmax, vmax]^3 (the
+    paper's electron grids: 36^3 on +-20 v_A at m_i/m_e = 100), thermal spread
+    sqrt(mass_ratio * temp_ratio) (T_e / T_i = temp_ratio), sheet drift -temp_ratio * drift (the Harris
+    equilibrium splits the current as the temperatures), its own seed."""
+    return replace(w, name=w.name + f"_electrons_{nv}^3", nv=(nv, nv, nv), vlo=(-vmax,) * 3, vhi=(vmax,) * 3,
+                   q_over_m=-mass_ratio, sigma=float(np.sqrt(mass_ratio * temp_ratio)),
+                   drift=-temp_ratio * w.drift, seed_offset=w.seed_offset + 500)
+
+
+def yee_fields(w: Workload):
+    """Seeded STAGGERED E, B (shape (3, nz, ny, nx) each, the lattice R19 of DESIGN.md) for coupled runs: the
+    Harris profile B_x = tanh(y / 0.5) (double sheet for harris3d) sampled at the positions of B_x on the lattice
+    plus the 1e-2 smooth perturbation, guide field, E = 1e-2 smooth noise; zero fields for landau1d."""
+    rng = np.random.default_rng(w.seed + 104729)
+    E = np.zeros((3,) + w.space_shape)
+    B = np.zeros((3,) + w.space_shape)
+    if w.kind == "landau1d":
+        return E, B
+    y_edge = w.x_centres(1) + 0.5 * w.dx(1)                       # B_x sits at (i, j + 1/2, k + 1/2)
+    if w.kind == "harris2d":
+        prof = np.tanh(y_edge / 0.5)
+    else:
+        prof = np.tanh((y_edge + 3.2) / 0.5) - np.tanh((y_edge - 3.2) / 0.5) - 1.0
+    B[0] = prof[None, :, None] + 1e-2 * _smooth_noise(w, rng)
+    B[2] = w.guide_bz
+    for a in range(3):
+        E[a] = 1e-2 * _smooth_noise(w, rng)
+    return np.ascontiguousarray(E), np.ascontiguousarray(B)

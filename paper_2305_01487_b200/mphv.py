@@ -28,6 +28,11 @@ SYMBOLS = (
     "mphv_set_fusion", "mphv_set_vmode", "mphv_maxwellian", "mphv_exchange_maxwellian", "mphv_match_moments", "mphv_strerror", "mphv_last_error",
     "mphv_set_timing", "mphv_timing_slots", "mphv_get_timing", "mphv_get_timing_moved",
     "mphv_stage_x", "mphv_stage_x_halo", "mphv_stage_v", "mphv_halo_count", "mphv_pack_halo", "mphv_sweep_x_halo",
+    "mphv_set_fields_deferred", "mphv_deferred_status",
+    "mphv_maxwell_create", "mphv_maxwell_destroy", "mphv_maxwell_set_stream", "mphv_maxwell_bind", "mphv_maxwell_faraday",
+    "mphv_maxwell_ampere", "mphv_maxwell_step", "mphv_maxwell_centre", "mphv_maxwell_current", "mphv_maxwell_last_error",
+    "mphv_plasma_create", "mphv_plasma_destroy", "mphv_plasma_set_concurrent", "mphv_plasma_step", "mphv_plasma_sync",
+    "mphv_plasma_moments", "mphv_plasma_centred_fields", "mphv_plasma_last_error",
 )
 
 
@@ -44,6 +49,11 @@ class mphv_grid(C.Structure):
 class mphv_box(C.Structure):
     _fields_ = [("xlo", C.c_double * 3), ("xhi", C.c_double * 3),
                 ("vlo", C.c_double * 3), ("vhi", C.c_double * 3)]
+
+
+class mphv_field_grid(C.Structure):
+    _fields_ = [("nx", C.c_int32 * 3), ("bc", C.c_int32 * 3), ("dx", C.c_double * 3),
+                ("c2", C.c_double), ("inv_eps0", C.c_double)]
 
 
 _lib = None
@@ -93,6 +103,26 @@ def lib() -> C.CDLL:
         "mphv_sweep_x_halo": (i32, [vp, i32, dbl, vp, vp]),
         "mphv_strerror": (C.c_char_p, [i32]),
         "mphv_last_error": (C.c_char_p, [vp]),
+        "mphv_set_fields_deferred": (i32, [vp, vp, vp]),
+        "mphv_deferred_status": (i32, [vp]),
+        "mphv_maxwell_create": (vp, [C.POINTER(mphv_field_grid)]),
+        "mphv_maxwell_destroy": (i32, [vp]),
+        "mphv_maxwell_set_stream": (i32, [vp, vp]),
+        "mphv_maxwell_bind": (i32, [vp, vp, vp]),
+        "mphv_maxwell_faraday": (i32, [vp, dbl]),
+        "mphv_maxwell_ampere": (i32, [vp, vp, dbl]),
+        "mphv_maxwell_step": (i32, [vp, vp, dbl]),
+        "mphv_maxwell_centre": (i32, [vp, vp, vp]),
+        "mphv_maxwell_current": (i32, [vp, i32, C.POINTER(dbl), C.POINTER(vp), vp]),
+        "mphv_maxwell_last_error": (C.c_char_p, [vp]),
+        "mphv_plasma_create": (vp, [vp, i32, C.POINTER(vp), C.POINTER(dbl)]),
+        "mphv_plasma_destroy": (i32, [vp]),
+        "mphv_plasma_set_concurrent": (i32, [vp, i32]),
+        "mphv_plasma_step": (i32, [vp, dbl, i32]),
+        "mphv_plasma_sync": (i32, [vp]),
+        "mphv_plasma_moments": (i32, [vp, i32, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]),
+        "mphv_plasma_centred_fields": (i32, [vp, C.POINTER(vp), C.POINTER(vp)]),
+        "mphv_plasma_last_error": (C.c_char_p, [vp]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)
@@ -265,6 +295,115 @@ def mphv_get_timing_moved(ctx, slot: int) -> float:
     return b.value
 
 
+# ---- fields and coupled step (include/mphv.h "closing the loop")
+def _check_m(m, st: int):
+    if st != OK:
+        raise MphvError(st, f"{mphv_strerror(st)}: {mphv_maxwell_last_error(m)}")
+
+
+def _check_p(p, st: int):
+    if st != OK:
+        raise MphvError(st, f"{mphv_strerror(st)}: {mphv_plasma_last_error(p)}")
+
+
+def mphv_set_fields_deferred(ctx, E_dev: int, B_dev: int):
+    _check(ctx, lib().mphv_set_fields_deferred(ctx, E_dev, B_dev))
+
+
+def mphv_deferred_status(ctx):
+    _check(ctx, lib().mphv_deferred_status(ctx))
+
+
+def mphv_maxwell_create(nx, bc, dx, c2: float = 1.0, inv_eps0: float = 1.0):
+    g = mphv_field_grid((C.c_int32 * 3)(*nx), (C.c_int32 * 3)(*bc), (C.c_double * 3)(*dx), float(c2), float(inv_eps0))
+    m = lib().mphv_maxwell_create(C.byref(g))
+    if not m:
+        raise MphvError(ERR_ARG, "mphv_maxwell_create failed: " + mphv_last_error(None))
+    return m
+
+
+def mphv_maxwell_destroy(m):
+    _check_m(None, lib().mphv_maxwell_destroy(m))
+
+
+def mphv_maxwell_set_stream(m, cuda_stream: int):
+    _check_m(m, lib().mphv_maxwell_set_stream(m, cuda_stream))
+
+
+def mphv_maxwell_bind(m, E_dev: int, B_dev: int):
+    _check_m(m, lib().mphv_maxwell_bind(m, E_dev, B_dev))
+
+
+def mphv_maxwell_faraday(m, dt: float):
+    _check_m(m, lib().mphv_maxwell_faraday(m, float(dt)))
+
+
+def mphv_maxwell_ampere(m, J_dev, dt: float):
+    _check_m(m, lib().mphv_maxwell_ampere(m, J_dev, float(dt)))
+
+
+def mphv_maxwell_step(m, J_dev, dt: float):
+    _check_m(m, lib().mphv_maxwell_step(m, J_dev, float(dt)))
+
+
+def mphv_maxwell_centre(m, Ec_dev: int, Bc_dev: int):
+    _check_m(m, lib().mphv_maxwell_centre(m, Ec_dev, Bc_dev))
+
+
+def mphv_maxwell_current(m, q: Sequence[float], j_dev_ptrs: Sequence[int], J_dev: int):
+    n = len(q)
+    qa = (C.c_double * n)(*map(float, q))
+    ja = (C.c_void_p * n)(*j_dev_ptrs)
+    _check_m(m, lib().mphv_maxwell_current(m, n, qa, ja, J_dev))
+
+
+def mphv_maxwell_last_error(m=None) -> str:
+    return lib().mphv_maxwell_last_error(m).decode()
+
+
+def mphv_plasma_create(m, species_ctx: Sequence, q: Sequence[float]):
+    n = len(species_ctx)
+    sa = (C.c_void_p * n)(*species_ctx)
+    qa = (C.c_double * n)(*map(float, q))
+    p = lib().mphv_plasma_create(m, n, sa, qa)
+    if not p:
+        raise MphvError(ERR_ARG, "mphv_plasma_create failed: " + mphv_last_error(None))
+    return p
+
+
+def mphv_plasma_destroy(p):
+    _check_p(None, lib().mphv_plasma_destroy(p))
+
+
+def mphv_plasma_set_concurrent(p, concurrent: bool):
+    _check_p(p, lib().mphv_plasma_set_concurrent(p, 1 if concurrent else 0))
+
+
+def mphv_plasma_step(p, dt: float, nsteps: int = 1):
+    _check_p(p, lib().mphv_plasma_step(p, float(dt), int(nsteps)))
+
+
+def mphv_plasma_sync(p):
+    _check_p(p, lib().mphv_plasma_sync(p))
+
+
+def mphv_plasma_moments(p, s: int):
+    """Device pointers (n, j, P) of the latest moments of species s."""
+    n, j, P = C.c_void_p(), C.c_void_p(), C.c_void_p()
+    _check_p(p, lib().mphv_plasma_moments(p, int(s), C.byref(n), C.byref(j), C.byref(P)))
+    return n.value, j.value, P.value
+
+
+def mphv_plasma_centred_fields(p):
+    Ec, Bc = C.c_void_p(), C.c_void_p()
+    _check_p(p, lib().mphv_plasma_centred_fields(p, C.byref(Ec), C.byref(Bc)))
+    return Ec.value, Bc.value
+
+
+def mphv_plasma_last_error(p=None) -> str:
+    return lib().mphv_plasma_last_error(p).decode()
+
+
 # ------------------------------------------------------------------ torch convenience
 class Vlasov:
     """One species on one GPU. Holds the context and references to the bound tensors."""
@@ -320,6 +459,14 @@ class Vlasov:
         ns = mphv_space_count(self.ctx)
         mphv_set_fields(self.ctx, self._dev(E, 3 * ns), self._dev(B, 3 * ns))
         self.E, self.B = E, B
+
+    def set_fields_deferred(self, E, B):
+        ns = mphv_space_count(self.ctx)
+        mphv_set_fields_deferred(self.ctx, self._dev(E, 3 * ns), self._dev(B, 3 * ns))
+        self.E, self.B = E, B
+
+    def deferred_status(self):
+        mphv_deferred_status(self.ctx)
 
     def sweep_x(self, dim, dt):
         mphv_sweep_x(self.ctx, dim, dt)
@@ -440,3 +587,120 @@ class Vlasov:
             if n:
                 out[name] = dict(ms=ms, launches=n, alg_bytes=b, moved_bytes=mphv_get_timing_moved(self.ctx, s))
         return out
+
+
+def _from_ptr(torch, ptr: int, shape, device, keep):
+    """A float64 torch view of library-owned device memory (no copy); `keep` is held so the owner outlives it."""
+    n = 1
+    for e in shape:
+        n *= int(e)
+
+    class _Mem:
+        __cuda_array_interface__ = {"shape": (n,), "typestr": "<f8", "data": (int(ptr), False), "version": 2}
+    t = torch.as_tensor(_Mem(), device=device).view(*shape)
+    t._mphv_owner = keep
+    return t
+
+
+class Maxwell:
+    """FDTD field solver on the Vlasov cells (readings R19..R21): staggered E, B as [3][nz][ny][nx] tensors."""
+
+    def __init__(self, nx, bc, dx, c2=1.0, inv_eps0=1.0, device="cuda:0"):
+        import torch
+        self.torch, self.device = torch, torch.device(device)
+        self.nx = tuple(nx)
+        self.ns = int(nx[0]) * int(nx[1]) * int(nx[2])
+        self.shape = (3, nx[2], nx[1], nx[0])
+        with torch.cuda.device(self.device):
+            self.m = mphv_maxwell_create(nx, bc, dx, c2, inv_eps0)
+        self.E = self.B = None
+
+    @classmethod
+    def from_workload(cls, w, c2=1.0, inv_eps0=1.0, **kw):
+        return cls(w.nx, w.bc, tuple(w.dx(d) if w.nx[d] > 1 else 1.0 for d in range(3)), c2, inv_eps0, **kw)
+
+    def _dev(self, t, count=None):
+        torch = self.torch
+        count = 3 * self.ns if count is None else count
+        if t.dtype != torch.float64 or not t.is_contiguous() or t.numel() != count or t.device != self.device:
+            raise ValueError(f"need a contiguous float64 tensor of {count} elements on {self.device}")
+        return t.data_ptr()
+
+    def close(self):
+        if self.m:
+            mphv_maxwell_destroy(self.m)
+            self.m = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def bind(self, E, B):
+        mphv_maxwell_bind(self.m, self._dev(E), self._dev(B))
+        self.E, self.B = E, B
+
+    def faraday(self, dt):
+        mphv_maxwell_faraday(self.m, dt)
+
+    def ampere(self, J, dt):
+        mphv_maxwell_ampere(self.m, None if J is None else self._dev(J), dt)
+
+    def step(self, J, dt):
+        mphv_maxwell_step(self.m, None if J is None else self._dev(J), dt)
+
+    def centre(self, out=None):
+        torch = self.torch
+        Ec, Bc = out if out is not None else (torch.empty(self.shape, dtype=torch.float64, device=self.device),
+                                              torch.empty(self.shape, dtype=torch.float64, device=self.device))
+        mphv_maxwell_centre(self.m, self._dev(Ec), self._dev(Bc))
+        return Ec, Bc
+
+    def current(self, q, j_list, out=None):
+        torch = self.torch
+        J = out if out is not None else torch.empty(self.shape, dtype=torch.float64, device=self.device)
+        mphv_maxwell_current(self.m, q, [self._dev(j) for j in j_list], self._dev(J))
+        return J
+
+
+class Plasma:
+    """Kinetic species coupled through Maxwell's equations (mphv_plasma_*): the coupled step R22."""
+
+    def __init__(self, maxwell: Maxwell, species: Sequence[Vlasov], q: Sequence[float]):
+        self.maxwell, self.species = maxwell, list(species)
+        self.torch, self.device = maxwell.torch, maxwell.device
+        with self.torch.cuda.device(self.device):
+            self.p = mphv_plasma_create(maxwell.m, [s.ctx for s in species], q)
+
+    def close(self):
+        if self.p:
+            mphv_plasma_destroy(self.p)
+            self.p = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_concurrent(self, concurrent: bool):
+        mphv_plasma_set_concurrent(self.p, concurrent)
+
+    def step(self, dt, nsteps=1):
+        mphv_plasma_step(self.p, dt, nsteps)
+
+    def sync(self):
+        mphv_plasma_sync(self.p)
+
+    def moments(self, s: int):
+        """(n, j, P) of species s as torch views of the plasma object's device buffers (call sync() first)."""
+        n, j, P = mphv_plasma_moments(self.p, s)
+        sp = self.maxwell.shape[1:]
+        return (_from_ptr(self.torch, n, sp, self.device, self), _from_ptr(self.torch, j, (3,) + sp, self.device, self),
+                _from_ptr(self.torch, P, (6,) + sp, self.device, self))
+
+    def centred_fields(self):
+        Ec, Bc = mphv_plasma_centred_fields(self.p)
+        return (_from_ptr(self.torch, Ec, self.maxwell.shape, self.device, self),
+                _from_ptr(self.torch, Bc, self.maxwell.shape, self.device, self))
