@@ -57,6 +57,9 @@ def parse():
     ap.add_argument("--aux", action="store_true",
                     help="instead of the step: time the coupling kernels of SURVEY 8(f) (ten-moment Maxwellian fill, "
                          "exchange of Maxwellians, moment matching) on the same workload and print one JSON line")
+    ap.add_argument("--no-two-species", action="store_true",
+                    help="skip the coupled two-species leg (ions + electrons + Maxwell, extra key two_species)")
+    ap.add_argument("--species-steps", type=int, default=6)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -452,6 +455,9 @@ def run_mphv(args, w):
                                     "what": "mphv_step_fields_host: f stays on the device; pinned host E, B -> device, "
                                             "set_fields, full split step, moments -> host, stream sync every step (wall clock)"}
 
+    if world == 1 and not halo_mode and not args.no_two_species and w.kind != "landau1d" and args.vmode == "plain":
+        line["two_species"] = run_two_species(args, torch, mphv, inputs, w, sim, f, dev)
+
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         del f0
         line["cpu_baseline"] = {k: v for k, v in time_oracle(w, 2, 1, args.cpu_seconds, adapt=True).items() if k != "ms_per_step"}
@@ -460,6 +466,48 @@ def run_mphv(args, w):
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
+
+
+def run_two_species(args, torch, mphv, inputs, w, ions, f_ions, dev):
+    """the paper's Scheme {Vlasov e, Vlasov i, Maxwell} on the workload's spatial grid.
+    Ions = the workload (f as the timed run left it), electrons = inputs.electrons_of (q/m = -100, 36^3 on +-20,
+    P:L215), FDTD Maxwell with c = 20; mphv_plasma_step (coupled step R22: per step 2 launches per species + 1
+    field launch, no host sync). Timed serially (everything on one stream) and with one stream per species; the
+    ratio says whether the SMs co-schedule one species' HBM-bound spatial sweeps with the other's issue-bound
+    V stage. dt = half the CFL bound over both species' sweeps."""
+    we = inputs.electrons_of(w)
+    fe = torch.from_numpy(inputs.make_f0(we)).to(dev)
+    Ey, By = inputs.yee_fields(w)
+    dt = 0.5 * min(inputs.cfl_dt(w, 2 * Ey, 2 * By), inputs.cfl_dt(we, 2 * Ey, 2 * By))
+    el = mphv.Vlasov.from_workload(we, device=dev)
+    el.bind_f(fe)
+    mx = mphv.Maxwell.from_workload(w, c2=400.0, inv_eps0=1.0, device=dev)
+    Ed, Bd = torch.from_numpy(Ey).to(dev), torch.from_numpy(By).to(dev)
+    mx.bind(Ed, Bd)
+    pl = mphv.Plasma(mx, [ions, el], [1.0, -1.0])
+    cells = w.n_cells + we.n_cells
+    steps = max(2, args.species_steps)
+    out = {"what": "mphv_plasma_step: ions (the workload) + electrons (%s, q/m = -100) + FDTD Maxwell, coupled step R22; "
+                   "value = cells of both species x steps / time (CUDA events on the field stream, which joins the species' streams)" % we.name,
+           "cells": {"ions": w.n_cells, "electrons": we.n_cells}, "steps": steps, "unit": UNIT}
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for mode in ("serial", "concurrent"):
+        pl.set_concurrent(mode == "concurrent")
+        pl.step(dt, 2)
+        pl.sync()
+        l0 = ions.launches + el.launches
+        e0.record()
+        pl.step(dt, steps)
+        e1.record()
+        pl.sync()
+        ms = e0.elapsed_time(e1)
+        out[mode] = {"ms_per_step": ms / steps, "value": cells * steps / (ms * 1e-3),
+                     "species_launches_per_step": (ions.launches + el.launches - l0) / steps}
+    out["speedup_concurrent_over_serial"] = out["serial"]["ms_per_step"] / out["concurrent"]["ms_per_step"]
+    n_i = pl.moments(0)[0]
+    assert bool(torch.isfinite(n_i).all()) and bool(torch.isfinite(Ed).all()) and float(fe.min()) >= 0.0
+    pl.close()
+    return out
 
 
 def run_aux(args, w):

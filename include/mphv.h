@@ -308,11 +308,15 @@ const char *mphv_maxwell_last_error(const mphv_maxwell *m);
  *        J = sum_s q_s j_s[f_s];  Maxwell(dt/2; J);  E_c, B_c = centred fields;
  *        every species: f_s <- mphv_step(dt) with E_c, B_c frozen, moments of the new f_s;
  *        J' = sum_s q_s j_s[f_s];  Maxwell(dt/2; J').
- * Every species runs on a CUDA stream of its own (concurrent = 1) so that one species' HBM-bound spatial sweeps can
- * overlap another's issue-bound V stage, the field update on a third; they are ordered by events, the host never
- * waits inside the loop (velocity RANGE checks are deferred, see mphv_set_fields_deferred). concurrent = 0 runs
- * everything on one stream (for comparison). The call returns after the last step has been enqueued and the streams
- * have been joined on the field solver's stream; mphv_plasma_sync waits for it and reports a deferred RANGE error.
+ * By default everything is enqueued on the field solver's stream (mphv_maxwell_set_stream). With
+ * mphv_plasma_set_concurrent(p, 1) every species runs on a CUDA stream of its own, ordered against the field update
+ * by events. Measured on B200 (profiles/r02b_two_species.md) that is SLOWER (7.05 vs 6.56 ms per step for ions
+ * 40^3 + electrons 36^3 on 128x64): the spatial-sweep kernel and the V-stage kernel each fill an SM's register file,
+ * so two species never share an SM, and two spatial sweeps at once split the L2 their row rings live in. Either way
+ * the host never waits inside the loop (velocity RANGE checks are deferred, see mphv_set_fields_deferred). The call
+ * returns after the last step has been enqueued (the species' streams joined on the field solver's stream);
+ * mphv_plasma_sync waits for it and reports a deferred RANGE error. The species contexts are left on the streams
+ * the last call used.
  * The first call computes the moments of the initial f_s itself.
  * mphv_plasma_moments: device pointers to the latest moments of species s (n [ns], j [3][ns], P [6][ns], owned by
  * the plasma object, valid after mphv_plasma_sync). */

@@ -274,7 +274,7 @@ mphv_plasma *mphv_plasma_create(mphv_maxwell *m, int nspecies, mphv_ctx *const *
     mphv_plasma *p = new (std::nothrow) mphv_plasma;
     if (!p) { fail_create("out of host memory"); return nullptr; }
     std::memset(p, 0, sizeof *p);
-    p->m = m; p->ns_species = nspecies; p->ns = (size_t)m->gd.ns; p->dev = m->dev; p->concurrent = 1;
+    p->m = m; p->ns_species = nspecies; p->ns = (size_t)m->gd.ns; p->dev = m->dev; p->concurrent = 0;
     DevGuard2 dg(p->dev);
     for (int s = 0; s < nspecies; ++s) { p->sp[s] = species[s]; p->q[s] = q[s]; }
     cudaError_t e = cudaMalloc(&p->buf, ((size_t)nspecies * 10 + 9) * p->ns * sizeof(double));
