@@ -436,7 +436,8 @@ def run_mphv(args, w):
                        "ms_per_step": ems / args.e2e_steps, "steps": args.e2e_steps,
                        "what": ("pinned host f -> device, decomposed split step with halo exchange, moments, f and moments -> host"
                                 if halo_mode else
-                                "mphv_run_host: pinned host f -> device, full split step, moments, f and moments -> host")}
+                                "mphv_run_host: pinned host f -> device, full split step, moments, f and moments -> host; the library cuts f "
+                                "into slabs along y and overlaps copy in, sweeps and copy out slab by slab")}
         del fh
         if not halo_mode:
             # coupled run, f resident: per step the host hands over E, B and gets n, j, P back

@@ -22,6 +22,19 @@
 
 using namespace mphv;
 
+// slab pipeline of mphv_run_host (see pipe_step)
+struct HostPipe {
+    int axis, K;
+    std::vector<mphv_ctx *> sub;
+    std::vector<int> row0;                    // first index of slab k along axis; row0[K] = n
+    double *halo;                             // [K][2 sides][halo_count of the thickest slab]
+    double *fld;                              // [K] x ([3][ns_k] E | [3][ns_k] B)
+    double *mom;                              // [10][ns_k max]
+    size_t halo_stride, layer;                // doubles per (slab, side); cells per index along axis
+    cudaStream_t h2d, d2h;
+    std::vector<cudaEvent_t> ev_in, ev_out;
+};
+
 struct mphv_ctx {
     mphv_grid grid;
     mphv_box box;
@@ -48,6 +61,7 @@ struct mphv_ctx {
     int vmode;                                       // 0 plain V sweeps, 1 backsubstitution
     double *bs_K;                                    // device [ns][12] face-displacement coefficients + [3] maxima
     double bs_dt; bool bs_valid; double bs_smax[3];
+    struct HostPipe *pipe;   // slab pipeline of mphv_run_host (lazy)
     uint64_t launches;
     int fusion;
     int timing;
@@ -652,6 +666,194 @@ int range_v(mphv_ctx *c, int d, double dt)
     return MPHV_OK;
 }
 
+
+// spatial sweeps along the axes below dmax, in order (dmax = 3: the whole X stage)
+int x_stage(mphv_ctx *c, double dt, int dmax = 3)
+{
+    int st;
+    int d0 = 0;
+    if (dmax >= 2 && c->fusion >= 3 && c->sxy_T > 0 && max_courant_x(c, 0, dt) < 1.0 && max_courant_x(c, 1, dt) < 1.0) {
+        if ((st = launch_sxy(c, dt)) != MPHV_OK) return st;        // S_x, S_y in one pass
+        d0 = 2;
+    }
+    for (int d = d0; d < dmax; ++d)
+        if (c->grid.nx[d] > 1 && (st = do_sweep_x(c, d, dt)) != MPHV_OK) return st;
+    return MPHV_OK;
+}
+
+
+// ---- mphv_run_host as a slab pipeline ---------------------------------------------------------------
+// f crosses PCIe both ways in one call; the step itself is ~40x shorter than either copy. The grid is cut
+// into K slabs along its outermost active spatial axis (contiguous in memory); slab k is swept while slab
+// k + 1 is still arriving and slab k - 1 is already leaving, so a call costs about max(H2D, D2H) instead of
+// their sum. Every slab is a block of a spatial decomposition: sweeps along the lower axes and
+// the V stage are local to it; the sweep along the slab axis takes its two ghost layers from the packed
+// boundary layers of the neighbouring slabs (pack_halo_kernel, march2_kernel<BC_HALO>), packed AFTER the
+// lower-axis sweeps of that slab and BEFORE its own slab-axis sweep overwrites them -- the order of the
+// multi-GPU path (halo.py). Result: that of mphv_step on the whole grid up to fp64 rounding.
+
+void destroy_pipe(mphv_ctx *c)
+{
+    HostPipe *hp = c->pipe;
+    if (!hp) return;
+    for (mphv_ctx *s : hp->sub) if (s) mphv_destroy(s);
+    for (cudaEvent_t e : hp->ev_in) if (e) cudaEventDestroy(e);
+    for (cudaEvent_t e : hp->ev_out) if (e) cudaEventDestroy(e);
+    if (hp->h2d) cudaStreamDestroy(hp->h2d);
+    if (hp->d2h) cudaStreamDestroy(hp->d2h);
+    if (hp->halo) cudaFree(hp->halo);
+    if (hp->fld) cudaFree(hp->fld);
+    if (hp->mom) cudaFree(hp->mom);
+    cudaGetLastError();
+    delete hp;
+    c->pipe = nullptr;
+}
+
+// builds the slab contexts once; false = this grid is not pipelined (the caller takes the plain path)
+bool ensure_pipe(mphv_ctx *c)
+{
+    if (c->pipe) return true;
+    int axis = -1;
+    for (int d = 2; d >= 0; --d) if (c->grid.nx[d] > 1) { axis = d; break; }
+    if (axis < 0) return false;
+    const int n = c->grid.nx[axis];
+    int K = n / 4 < 16 ? n / 4 : 16;
+    if (K < 3 || c->nf * sizeof(double) < (size_t)16 << 20) return false;      // small problems: not worth it
+    HostPipe *hp = new (std::nothrow) HostPipe();
+    if (!hp) return false;
+    c->pipe = hp;
+    hp->axis = axis; hp->K = K;
+    hp->halo = hp->fld = hp->mom = nullptr; hp->h2d = hp->d2h = nullptr;
+    hp->layer = c->nf / (size_t)n;
+    hp->row0.resize(K + 1);
+    for (int k = 0; k <= K; ++k) hp->row0[k] = (int)((long long)n * k / K);
+    hp->sub.assign(K, nullptr); hp->ev_in.assign(K, nullptr); hp->ev_out.assign(K, nullptr);
+    bool ok = cudaStreamCreateWithFlags(&hp->h2d, cudaStreamNonBlocking) == cudaSuccess &&
+              cudaStreamCreateWithFlags(&hp->d2h, cudaStreamNonBlocking) == cudaSuccess;
+    size_t nsk_max = 0;
+    for (int k = 0; k < K && ok; ++k) {
+        mphv_grid g = c->grid;
+        mphv_box b = c->box;
+        const int nk = hp->row0[k + 1] - hp->row0[k];
+        g.nx[axis] = nk;
+        b.xlo[axis] = c->box.xlo[axis] + c->dx[axis] * hp->row0[k];
+        b.xhi[axis] = c->box.xlo[axis] + c->dx[axis] * hp->row0[k + 1];
+        mphv_ctx *s = mphv_create(&g, &b, c->qm);
+        ok = s != nullptr;
+        if (!ok) break;
+        s->dx[axis] = c->dx[axis];                       // bitwise the parent's cell width (Courant numbers)
+        hp->sub[k] = s;
+        if (s->ns > nsk_max) nsk_max = s->ns;
+        ok = cudaEventCreateWithFlags(&hp->ev_in[k], cudaEventDisableTiming) == cudaSuccess &&
+             cudaEventCreateWithFlags(&hp->ev_out[k], cudaEventDisableTiming) == cudaSuccess;
+    }
+    if (ok) {
+        hp->halo_stride = 2 * hp->layer;
+        ok = cudaMalloc(&hp->halo, (size_t)K * 2 * hp->halo_stride * sizeof(double)) == cudaSuccess &&
+             cudaMalloc(&hp->fld, 6 * c->ns * sizeof(double)) == cudaSuccess &&
+             cudaMalloc(&hp->mom, 10 * nsk_max * sizeof(double)) == cudaSuccess;
+    }
+    if (!ok) { cudaGetLastError(); destroy_pipe(c); return false; }
+    return true;
+}
+
+// One full split step of the bound f, slab by slab. f_in: host source of f (NULL: f is already on the device);
+// f_out: host destination (NULL: f stays); mn/mj/mP: full-grid moment arrays on the device or NULL.
+int pipe_step(mphv_ctx *c, double dt, const double *f_in, double *f_out, double *mn, double *mj, double *mP)
+{
+    HostPipe *hp = c->pipe;
+    const int K = hp->K, axis = hp->axis;
+    const bool periodic = c->grid.bc[axis] == MPHV_BC_PERIODIC;
+    int st;
+    // per-slab views of f and of the fields ([3][ns_k] blocks cut out of the parent's [3][ns])
+    size_t off_cells = 0;
+    for (int k = 0; k < K; ++k) {
+        mphv_ctx *s = hp->sub[k];
+        s->stream = c->stream; s->fusion = c->fusion; s->timing = 0; s->vmode = 0;
+        s->f = c->f + (size_t)hp->row0[k] * hp->layer; s->scratch = nullptr;
+        double *Ek = hp->fld + 6 * off_cells, *Bk = Ek + 3 * s->ns;
+        CUDA_TRY(c, cudaMemcpy2DAsync(Ek, s->ns * sizeof(double), c->E + off_cells, c->ns * sizeof(double), s->ns * sizeof(double), 3, cudaMemcpyDeviceToDevice, c->stream));
+        CUDA_TRY(c, cudaMemcpy2DAsync(Bk, s->ns * sizeof(double), c->B + off_cells, c->ns * sizeof(double), s->ns * sizeof(double), 3, cudaMemcpyDeviceToDevice, c->stream));
+        s->E = Ek; s->B = Bk; s->deferred = false;
+        for (int d = 0; d < 3; ++d) s->amax[d] = c->amax[d];          // the parent's bound covers every slab
+        off_cells += s->ns;
+    }
+    if (f_in) {
+        cudaEvent_t ready = hp->ev_out[0];               // f must be free (earlier work on the compute stream done)
+        CUDA_TRY(c, cudaEventRecord(ready, c->stream));
+        CUDA_TRY(c, cudaStreamWaitEvent(hp->h2d, ready, 0));
+        for (int k = 0; k < K; ++k) {
+            const size_t o = (size_t)hp->row0[k] * hp->layer, cnt = hp->sub[k]->nf;
+            CUDA_TRY(c, cudaMemcpyAsync(c->f + o, f_in + o, cnt * sizeof(double), cudaMemcpyHostToDevice, hp->h2d));
+            CUDA_TRY(c, cudaEventRecord(hp->ev_in[k], hp->h2d));
+        }
+    }
+    auto lo_buf = [&](int k) { return hp->halo + (size_t)(2 * k) * hp->halo_stride; };       // packed LOW layers of slab k
+    auto hi_buf = [&](int k) { return hp->halo + (size_t)(2 * k + 1) * hp->halo_stride; };   // packed HIGH layers of slab k
+    // lower-axis sweeps of slab k, then its two boundary layers packed for the neighbours
+    auto stage_local = [&](int k) -> int {
+        mphv_ctx *s = hp->sub[k];
+        if (f_in) CUDA_TRY(c, cudaStreamWaitEvent(c->stream, hp->ev_in[k], 0));
+        int e = x_stage(s, dt, axis);
+        if (e != MPHV_OK) return e;
+        if ((e = mphv_pack_halo(s, axis, 0, lo_buf(k))) != MPHV_OK) return e;
+        return mphv_pack_halo(s, axis, 1, hi_buf(k));
+    };
+    // slab-axis sweep with the neighbours' layers, V stage, moments, and the way out
+    auto stage_rest = [&](int k) -> int {
+        mphv_ctx *s = hp->sub[k];
+        const double *lo = k > 0 ? hi_buf(k - 1) : (periodic ? hi_buf(K - 1) : nullptr);
+        const double *hi = k + 1 < K ? lo_buf(k + 1) : (periodic ? lo_buf(0) : nullptr);
+        MarchArgs a = march_args_space(s, axis, dt);
+        a.halo_lo = lo; a.halo_hi = hi;
+        int e = launch_march<KIND_SPACE, BC_HALO>(s, a);
+        if (e != MPHV_OK) return e;
+        if (mn) {
+            double *tn = hp->mom, *tj = tn + s->ns, *tP = tn + 4 * s->ns;
+            if ((e = do_v_stage(s, dt, tn, tj, tP)) != MPHV_OK) return e;
+            const size_t o = (size_t)hp->row0[k] * (c->ns / (size_t)c->grid.nx[axis]);
+            const size_t w = s->ns * sizeof(double), dp = c->ns * sizeof(double);
+            CUDA_TRY(c, cudaMemcpyAsync(mn + o, tn, w, cudaMemcpyDeviceToDevice, c->stream));
+            CUDA_TRY(c, cudaMemcpy2DAsync(mj + o, dp, tj, w, w, 3, cudaMemcpyDeviceToDevice, c->stream));
+            CUDA_TRY(c, cudaMemcpy2DAsync(mP + o, dp, tP, w, w, 6, cudaMemcpyDeviceToDevice, c->stream));
+        } else if ((e = do_v_stage(s, dt, nullptr, nullptr, nullptr)) != MPHV_OK) return e;
+        if (f_out) {
+            const size_t o = (size_t)hp->row0[k] * hp->layer;
+            CUDA_TRY(c, cudaEventRecord(hp->ev_out[k], c->stream));
+            CUDA_TRY(c, cudaStreamWaitEvent(hp->d2h, hp->ev_out[k], 0));
+            CUDA_TRY(c, cudaMemcpyAsync(f_out + o, c->f + o, s->nf * sizeof(double), cudaMemcpyDeviceToHost, hp->d2h));
+        }
+        return MPHV_OK;
+    };
+    // order: local(0), local(1), rest(0) [outflow] ..., a periodic axis keeps slab 0 for last (it needs slab K-1)
+    if ((st = stage_local(0)) != MPHV_OK) return st;
+    for (int k = 1; k < K; ++k) {
+        if ((st = stage_local(k)) != MPHV_OK) return st;
+        if (k - 1 > 0 || !periodic) { if ((st = stage_rest(k - 1)) != MPHV_OK) return st; }
+    }
+    if (periodic) {
+        // slab K-1 needs lo_buf(0) (packed), slab 0 needs hi_buf(K-1) (packed): both are there now
+        if ((st = stage_rest(K - 1)) != MPHV_OK) return st;
+        if ((st = stage_rest(0)) != MPHV_OK) return st;
+    } else if ((st = stage_rest(K - 1)) != MPHV_OK) return st;
+    for (int k = 0; k < K; ++k) c->launches += hp->sub[k]->launches, hp->sub[k]->launches = 0;
+    if (f_out) {                                         // the compute stream's owner waits for the copies out
+        cudaEvent_t done = hp->ev_in[0];
+        CUDA_TRY(c, cudaEventRecord(done, hp->d2h));
+        CUDA_TRY(c, cudaStreamWaitEvent(c->stream, done, 0));
+    }
+    return MPHV_OK;
+}
+
+bool pipe_eligible(mphv_ctx *c, double dt)
+{
+    if (c->vmode || c->deferred) return false;
+    int axis = -1;
+    for (int d = 2; d >= 0; --d) if (c->grid.nx[d] > 1) { axis = d; break; }
+    if (axis < 0 || !(max_courant_x(c, axis, dt) < 1.0)) return false;      // halo sweeps need |s| < 1
+    return ensure_pipe(c);
+}
+
 }  // namespace
 
 extern "C" {
@@ -839,6 +1041,7 @@ int mphv_destroy(mphv_ctx *c)
     if (c->ws) cudaFree(c->ws);
     if (c->fld) cudaFree(c->fld);
     if (c->bs_K) cudaFree(c->bs_K);
+    destroy_pipe(c);
     if (c->pending) { drain_timing(c, false); delete c->pending; }
     delete c;
     return MPHV_OK;
@@ -956,19 +1159,6 @@ static int step_checks(mphv_ctx *c, double dt)
         if (c->grid.nx[d] > 1 && (st = range_x(c, d, dt)) != MPHV_OK) return st;
     for (int d = 0; d < 3; ++d)
         if (c->grid.nv[d] > 1 && (st = range_v(c, d, dt)) != MPHV_OK) return st;
-    return MPHV_OK;
-}
-
-static int x_stage(mphv_ctx *c, double dt)
-{
-    int st;
-    int d0 = 0;
-    if (c->fusion >= 3 && c->sxy_T > 0 && max_courant_x(c, 0, dt) < 1.0 && max_courant_x(c, 1, dt) < 1.0) {
-        if ((st = launch_sxy(c, dt)) != MPHV_OK) return st;        // S_x, S_y in one pass
-        d0 = 2;
-    }
-    for (int d = d0; d < 3; ++d)
-        if (c->grid.nx[d] > 1 && (st = do_sweep_x(c, d, dt)) != MPHV_OK) return st;
     return MPHV_OK;
 }
 
@@ -1150,14 +1340,25 @@ int mphv_run_host(mphv_ctx *c, double *f_host, int nsteps, double dt, double *n_
     int st = step_checks(c, dt);
     if (st != MPHV_OK) return st;
     if (!f_host || nsteps < 0) { set_err(c, "f_host is NULL or nsteps < 0"); return MPHV_ERR_ARG; }
-    CUDA_TRY(c, cudaMemcpyAsync(c->f, f_host, c->nf * sizeof(double), cudaMemcpyHostToDevice, c->stream));
     double *mn = ws_moments(c), *mj = mn + c->ns, *mP = mn + 4 * c->ns;
-    for (int s = 0; s + 1 < nsteps; ++s)
-        if ((st = mphv_step(c, dt)) != MPHV_OK) return st;
-    if (nsteps > 0) st = step_impl(c, dt, mn, mj, mP);       // last step with the moments fused in
-    else st = do_moments(c, mn, mj, mP);
-    if (st != MPHV_OK) return st;
-    CUDA_TRY(c, cudaMemcpyAsync(f_host, c->f, c->nf * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    if (nsteps > 0 && pipe_eligible(c, dt)) {
+        // slab pipeline: the first step overlaps the copy in, the last one the copy out (see HostPipe)
+        for (int s = 0; s < nsteps; ++s) {
+            const bool first = s == 0, last = s + 1 == nsteps;
+            if (first || last) st = pipe_step(c, dt, first ? f_host : nullptr, last ? f_host : nullptr,
+                                              last ? mn : nullptr, last ? mj : nullptr, last ? mP : nullptr);
+            else st = mphv_step(c, dt);
+            if (st != MPHV_OK) return st;
+        }
+    } else {
+        CUDA_TRY(c, cudaMemcpyAsync(c->f, f_host, c->nf * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+        for (int s = 0; s + 1 < nsteps; ++s)
+            if ((st = mphv_step(c, dt)) != MPHV_OK) return st;
+        if (nsteps > 0) st = step_impl(c, dt, mn, mj, mP);       // last step with the moments fused in
+        else st = do_moments(c, mn, mj, mP);
+        if (st != MPHV_OK) return st;
+        CUDA_TRY(c, cudaMemcpyAsync(f_host, c->f, c->nf * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    }
     if (n_host) CUDA_TRY(c, cudaMemcpyAsync(n_host, mn, c->ns * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     if (j_host) CUDA_TRY(c, cudaMemcpyAsync(j_host, mj, 3 * c->ns * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     if (P_host) CUDA_TRY(c, cudaMemcpyAsync(P_host, mP, 6 * c->ns * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
