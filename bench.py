@@ -307,6 +307,9 @@ def run_mphv(args, w):
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     if world > 1:
+        # NCCL's communicator log (ranks, transports, NVLS) on stderr, so that a run record shows the N ranks
+        os.environ.setdefault("NCCL_DEBUG", "INFO")
+        os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
         dist.init_process_group("nccl", device_id=dev)
     halo_mode = args.decomp == "halo" or (args.decomp == "auto" and world > 1)
     if halo_mode:

@@ -61,21 +61,35 @@ __device__ __forceinline__ double maxw_eval(const MaxwCoef &m, double vx, double
 enum { MAXW_RS = 8 };
 struct MaxwLine {
     double a0, b, e, r, rho;
-    __device__ __forceinline__ void init(const MaxwCoef &m, double vx, double vy, double dvz)
+    double czz, norm, uz;            // for the direct evaluation of a block the recurrence cannot carry
+    bool direct;
+    __device__ __forceinline__ void init(const MaxwCoef &m, double vx, double vy, double dvz_)
     {
         const double dx = vx - m.ux, dy = vy - m.uy;
         a0 = dx * (m.cxx * dx + m.cxy * dy) + m.cyy * dy * dy;
         b = m.cxz * dx + m.cyz * dy;
-        rho = exp(2.0 * m.czz * dvz * dvz);
+        rho = exp(2.0 * m.czz * dvz_ * dvz_);
         e = 0.0; r = 0.0;
+        czz = m.czz; norm = m.norm; uz = m.uz; direct = false;
     }
-    __device__ __forceinline__ void restart(const MaxwCoef &m, double vz, double dvz)
+    __device__ __forceinline__ void restart(const MaxwCoef &m, double vz, double dvz_)
     {
         const double dz = vz - m.uz;
         e = m.norm * exp(a0 + dz * (b + m.czz * dz));
-        r = exp(dvz * (b + m.czz * (2.0 * dz + dvz)));
+        r = exp(dvz_ * (b + m.czz * (2.0 * dz + dvz_)));
+        // A cold or unresolved Maxwellian (thermal spread << dvz): e underflows while r overflows and the
+        // recurrence would write 0 * inf = NaN, or lose the cells that come back above the underflow threshold
+        // inside the block. Such blocks are evaluated cell by cell (one exp each), like the definition.
+        direct = !(e > 1e-250 && r > 1e-25 && r < 1e25);
     }
+    // the value at the next cell of the pencil by the recurrence (only while !direct)
     __device__ __forceinline__ double next() { const double v = e; e *= r; r *= rho; return v; }
+    // the value at cell jz by the definition (one exp): what a block with `direct` set must use
+    __device__ __forceinline__ double eval(const GridDev &g, int jz) const
+    {
+        const double dz = vcentre(g, 2, jz) - uz;
+        return norm * exp(a0 + dz * (b + czz * dz));
+    }
 };
 
 struct MaxwArgs {
@@ -103,9 +117,17 @@ maxwellian_kernel(const MaxwArgs p)
         const double vx = vcentre(g, 0, jx), vy = vcentre(g, 1, jy);
         MaxwLine ln;
         ln.init(m, vx, vy, g.dv[2]);
-        for (int jz = 0; jz < g.nv[2]; ++jz) {
-            if (jz % MAXW_RS == 0) ln.restart(m, vcentre(g, 2, jz), g.dv[2]);
-            cube[(long long)jz * plane + pos] = m.norm > 0.0 ? ln.next() : 0.0;
+        for (int j0 = 0; j0 < g.nv[2]; j0 += MAXW_RS) {
+            ln.restart(m, vcentre(g, 2, j0), g.dv[2]);
+            if (ln.direct && m.norm > 0.0) {               // a cold Maxwellian: this block by the definition
+                for (int u = 0; u < MAXW_RS && j0 + u < g.nv[2]; ++u) cube[(long long)(j0 + u) * plane + pos] = ln.eval(g, j0 + u);
+                continue;
+            }
+#pragma unroll
+            for (int u = 0; u < MAXW_RS; ++u) {
+                const double v = m.norm > 0.0 ? ln.next() : 0.0;
+                if (j0 + u < g.nv[2]) cube[(long long)(j0 + u) * plane + pos] = v;
+            }
         }
     }
 }
@@ -187,6 +209,14 @@ exchange_kernel(const ExchArgs p)
             double fv[MAXW_RS];
 #pragma unroll
             for (int u = 0; u < MAXW_RS; ++u) fv[u] = j0 + u < g.nv[2] ? fext[(long long)(j0 + u) * plane + pos] : 0.0;
+            if (la.direct || lb.direct) {                  // a cold Maxwellian: this block by the definition
+                for (int u = 0; u < MAXW_RS && j0 + u < g.nv[2]; ++u) {
+                    const double a = mfl.norm > 0.0 ? la.eval(g, j0 + u) : 0.0;
+                    const double b = mex.norm > 0.0 ? lb.eval(g, j0 + u) : 0.0;
+                    dst[(long long)(j0 + u) * plane + pos] = a + sigma * (fv[u] - b);
+                }
+                continue;
+            }
 #pragma unroll
             for (int u = 0; u < MAXW_RS; ++u) {
                 const double a = mfl.norm > 0.0 ? la.next() : 0.0;
@@ -261,6 +291,14 @@ match_kernel(const MatchArgs p)
             double fv[MAXW_RS];
 #pragma unroll
             for (int u = 0; u < MAXW_RS; ++u) fv[u] = j0 + u < g.nv[2] ? cube[(long long)(j0 + u) * plane + pos] : 0.0;
+            if (la.direct || lb.direct) {                  // a cold Maxwellian: this block by the definition
+                for (int u = 0; u < MAXW_RS && j0 + u < g.nv[2]; ++u) {
+                    const double a = mt.norm > 0.0 ? la.eval(g, j0 + u) : 0.0;
+                    const double b = mf.norm > 0.0 ? lb.eval(g, j0 + u) : 0.0;
+                    cube[(long long)(j0 + u) * plane + pos] = a + (fv[u] - b);
+                }
+                continue;
+            }
 #pragma unroll
             for (int u = 0; u < MAXW_RS; ++u) {
                 const double a = mt.norm > 0.0 ? la.next() : 0.0;

@@ -164,6 +164,10 @@ class DistributedVlasov:
         self.decomp, self.rank = decomp, rank
         self.w = decomp.local_workload(w_global, rank)
         self.sim = mphv.Vlasov.from_workload(self.w, device=device)
+        # The kernels must run on the stream the process group's point-to-point calls are ordered against: NCCL
+        # work is enqueued behind the CURRENT torch stream, so the context follows it (checked again every step).
+        self._stream = None
+        self._follow_current_stream()
         self.xchg = HaloExchange(decomp, rank, group)
         self.buf = {}
         forced = (0, 1, 2) if force_halo is True else tuple(force_halo or ())
@@ -173,13 +177,25 @@ class DistributedVlasov:
                 cnt = self.sim.halo_count(d)
                 self.buf[d] = [torch.empty(cnt, dtype=torch.float64, device=self.sim.device) for _ in range(4)]
 
+    def _follow_current_stream(self):
+        torch = self.torch
+        if self.sim.device.type != "cuda":
+            return
+        cur = torch.cuda.current_stream(self.sim.device).cuda_stream
+        if cur != self._stream:
+            from . import mphv
+            mphv.mphv_set_stream(self.sim.ctx, cur or None)
+            self._stream = cur
+
     def bind_f(self, f, scratch=None):
         self.sim.bind_f(f, scratch)
 
     def set_fields(self, E, B):
+        self._follow_current_stream()
         self.sim.set_fields(E, B)
 
     def sweep_x(self, d: int, dt: float):
+        self._follow_current_stream()
         if not self.use_halo[d]:
             self.sim.sweep_x(d, dt)
             return
@@ -193,6 +209,7 @@ class DistributedVlasov:
         self.step_moments(dt, None)
 
     def step_moments(self, dt: float, out=None):
+        self._follow_current_stream()
         if self.use_halo[0] and not self.use_halo[1] and not self.use_halo[2]:
             # decomposed along x only: one exchange, then the whole X stage (S_x and S_y in one pass)
             send_lo, send_hi, recv_lo, recv_hi = self.buf[0]

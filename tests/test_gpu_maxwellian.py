@@ -55,6 +55,35 @@ def test_maxwellian_matches_oracle(torch_cuda, mphv, orc, nv):
         assert np.all(np.abs(got[c] - ref[c]) <= TOL * np.abs(ref[c]) + 1e-300), (c, _worst(got[c], ref[c]))
 
 
+@pytest.mark.parametrize("sigma", [0.05, 0.012, 0.3])
+def test_cold_maxwellians_have_no_nan(torch_cuda, mphv, orc, sigma):
+    """Thermal spread far below the cell width (dv = 0.31..1.25 here), centred near the box edge and in the middle:
+    the vz recurrence would form 0 * inf; such blocks are evaluated cell by cell. No NaN, and every element within
+    the relative bound (the oracle evaluates one exp per cell and underflows to 0 where the kernel must too)."""
+    torch = torch_cuda
+    w = small_workload((4, 4, 1), (16, 8, 32))
+    sim = mphv.Vlasov.from_workload(w)
+    grid, box = orc.Grid(w.nx, w.nv, w.bc), orc.Box(w.xlo, w.xhi, w.vlo, w.vhi)
+    n, j, P = [], [], []
+    for u in ((0.0, 0.0, 0.0), (0.0, 0.0, 0.02), (-0.01, 0.01, -0.03), (0.0, 0.02, 0.0)):      # small drifts: C = P/n - uu stays well conditioned
+        a, b, c = _moments_from(1.0, np.array(u), np.diag([sigma ** 2, (2 * sigma) ** 2, sigma ** 2]))
+        n.append(a); j.append(b); P.append(c)
+    n, j, P = np.array(n), np.array(j).T.copy(), np.array(P).T.copy()
+    ref = orc.maxwellian(grid, box, n, j, P)
+    got = sim.maxwellian(torch.from_numpy(n).cuda(), torch.from_numpy(j).cuda(), torch.from_numpy(P).cuda()).cpu().numpy()
+    assert np.isfinite(got).all()
+    assert np.all(np.abs(got - ref) <= TOL * np.abs(ref) + 1e-300), _worst(got, ref)
+    # and through the matching kernel, whose target moments come from the caller
+    f = np.abs(np.random.default_rng(5).standard_normal((4,) + ref.shape[1:])) + 0.1
+    wl = small_workload((4, 1, 1), (16, 8, 32))
+    sim2 = mphv.Vlasov.from_workload(wl)
+    fd = torch.from_numpy(f.reshape(wl.shape).copy()).cuda()
+    sim2.bind_f(fd)
+    sim2.match_moments(torch.from_numpy(n.reshape(1, 1, 4)).cuda(), torch.from_numpy(j.reshape(3, 1, 1, 4)).cuda(),
+                       torch.from_numpy(P.reshape(6, 1, 1, 4)).cuda())
+    assert bool(torch.isfinite(fd).all())
+
+
 @pytest.mark.parametrize("nx,dim", [((6, 4, 1), 0), ((4, 6, 1), 1), ((4, 4, 5), 2)])
 @pytest.mark.parametrize("side", [0, 1])
 def test_exchange_maxwellian_matches_oracle(torch_cuda, mphv, orc, nx, dim, side):
