@@ -7,6 +7,7 @@
 #include "mphv_march.cuh"
 #include "mphv_vstage.cuh"
 #include "mphv_vstage2.cuh"
+#include "mphv_vstage3.cuh"
 #include "mphv_sxy.cuh"
 #include "mphv_backsub.cuh"
 #include "mphv_vstage_bs.cuh"
@@ -54,6 +55,7 @@ struct mphv_ctx {
     int sm_count;
     int vxy_T, vxy_grid; size_t vxy_smem;     // fused V_vx + V_vy plane kernel launch shape (0 = unsupported)
     int vs_T, vs_grid, vs_variant, vs_bs; size_t vs_smem;
+    int vs3_T, vs3_grid; size_t vs3_smem;            // fourth-generation (warp-specialised) whole-V-stage kernel, plain mode (T = 0: shape not covered)
     int vs2_T, vs2_grid; size_t vs2_smem;            // third-generation whole-V-stage kernel, plain mode (T = 0: shape not covered)
     unsigned char vs_afirst[16], vs_acnt[16];         // stage-A warp items per warp of vstage_kernel (balance_stage_a)   // second-generation whole-V-stage kernel (T = 0: unsupported)
     int sxy_T, sxy_C; size_t sxy_smem;               // fused S_x + S_y kernel (T = 0: unsupported)
@@ -322,6 +324,31 @@ template <bool MOM> void *vstage2_fn(int variant)
     default:      return nullptr;
     }
 }
+// fourth-generation whole-V-stage kernel (mphv_vstage3.cuh), warp-specialised:
+// <ring depth, MOM, nvx, nvy, rows per patch, cells per run, B threads, launch threads, B registers, A registers>
+#ifndef MPHV_VS3_NS40
+#define MPHV_VS3_NS40 4
+#endif
+#ifndef MPHV_VS3_RB40
+#define MPHV_VS3_RB40 144
+#define MPHV_VS3_RA40 80
+#endif
+template <bool MOM> void *vstage3_fn(int variant)
+{
+    switch (variant) {
+    case CUBE_40: return (void *)vstage3_kernel<MPHV_VS3_NS40, MOM, 40, 40, 5, 20, 320, 512, MPHV_VS3_RB40, MPHV_VS3_RA40>;
+    // (32 x 32 planes: measured slower than vstage2_kernel, 0.72 vs 0.62 ms on c2 -- 8 B warps sit evenly on the schedulers there)
+    default:      return nullptr;
+    }
+}
+int vstage3_threads(int variant) { return variant == CUBE_40 ? 512 : 0; }
+int vstage3_ns(int variant) { return variant == CUBE_40 ? MPHV_VS3_NS40 : 4; }
+size_t vstage3_smem_bytes(int nvx, int nvy, int nvz, int ns)
+{
+    const size_t cells = (size_t)nvx * nvy, xcells = (size_t)nvx * (nvy + 4);
+    return (ns * 2 * cells + 4 * 2 * xcells + nvz + 320) * sizeof(double) + (2 * ns + 8) * sizeof(uint64_t);
+}
+
 int vstage2_threads(int variant) { return variant == CUBE_40 ? 320 : variant == CUBE_32 ? 256 : variant == CUBE_36 ? 224 : variant == CUBE_16 ? 64 : 0; }
 int vstage2_ns(int variant) { return variant == CUBE_40 ? MPHV_VS2_NS40 : 3; }
 size_t vstage2_smem_bytes(int nvx, int nvy, int nvz, int ns)
@@ -370,7 +397,8 @@ int launch_vcube(mphv_ctx *c, double dt, bool with_vz, double *n, double *j, dou
 // V_vx, V_vy, V_vz (+ moments if n != NULL) in one pass over f, two planes per pipeline iteration
 int launch_vstage(mphv_ctx *c, double dt, double *n, double *j, double *P, bool backsub = false)
 {
-    const bool gen3 = !backsub && c->vs2_T > 0;
+    const bool gen4 = !backsub && c->vs3_T > 0;
+    const bool gen3 = !backsub && !gen4 && c->vs2_T > 0;
     CubeArgs a;
     std::memset(&a, 0, sizeof a);
     a.f = c->f;
@@ -385,10 +413,12 @@ int launch_vstage(mphv_ctx *c, double dt, double *n, double *j, double *P, bool 
     Timed tm(c, n ? SLOT_VCUBE_MOM : SLOT_VCUBE, (n ? 56.0 : 48.0) * (double)c->nf, 16.0 * (double)c->nf);
     a.K = backsub ? c->bs_K : nullptr;
     void *fn = backsub ? (n ? vstage_bs_fn<true>(c->vs_variant) : vstage_bs_fn<false>(c->vs_variant))
+               : gen4  ? (n ? vstage3_fn<true>(c->vs_variant) : vstage3_fn<false>(c->vs_variant))
                : gen3  ? (n ? vstage2_fn<true>(c->vs_variant) : vstage2_fn<false>(c->vs_variant))
                        : (n ? vstage_fn<true>(c->vs_variant) : vstage_fn<false>(c->vs_variant));
     void *args[] = { &a };
-    cudaError_t e = gen3 ? cudaLaunchKernel(fn, dim3((unsigned)c->vs2_grid), dim3((unsigned)c->vs2_T), args, c->vs2_smem, c->stream)
+    cudaError_t e = gen4 ? cudaLaunchKernel(fn, dim3((unsigned)c->vs3_grid), dim3((unsigned)c->vs3_T), args, c->vs3_smem, c->stream)
+                  : gen3 ? cudaLaunchKernel(fn, dim3((unsigned)c->vs2_grid), dim3((unsigned)c->vs2_T), args, c->vs2_smem, c->stream)
                          : cudaLaunchKernel(fn, dim3((unsigned)c->vs_grid), dim3((unsigned)c->vs_T), args, c->vs_smem, c->stream);
     if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(c, e, "vstage_kernel launch"); }
     return after_launch(c, "vstage_kernel");
@@ -987,8 +1017,25 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
                        cudaFuncSetAttribute(vstage_bs_fn<false>(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess;
         }
         cudaGetLastError();
+        c->vs3_T = 0;
+        const char *gen_env = std::getenv("MPHV_VSTAGE_GEN");          // experiments: 2 / 3 force an older generation
+        const int gen_max = gen_env ? std::atoi(gen_env) : 4;
+        if (c->vs_T > 0 && gen_max >= 4 && vstage3_fn<true>(variant)) {
+            const size_t smem3 = vstage3_smem_bytes(nvx, nvy, nvz, vstage3_ns(variant));
+            const int T3 = vstage3_threads(variant);
+            int per3 = 0;
+            if (smem3 <= (size_t)max_optin &&
+                cudaFuncSetAttribute(vstage3_fn<true>(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem3) == cudaSuccess &&
+                cudaFuncSetAttribute(vstage3_fn<false>(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem3) == cudaSuccess &&
+                cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per3, vstage3_fn<true>(variant), T3, smem3) == cudaSuccess && per3 > 0) {
+                long long g3 = (long long)c->sm_count;
+                if (g3 > (long long)c->ns) g3 = (long long)c->ns;
+                c->vs3_T = T3; c->vs3_smem = smem3; c->vs3_grid = (int)g3;
+            }
+            cudaGetLastError();
+        }
         c->vs2_T = 0;
-        if (c->vs_T > 0 && vstage2_fn<true>(variant)) {
+        if (c->vs_T > 0 && gen_max >= 3 && vstage2_fn<true>(variant)) {
             const size_t smem2 = vstage2_smem_bytes(nvx, nvy, nvz, vstage2_ns(variant));
             const int T2 = vstage2_threads(variant);
             int per2 = 0;
