@@ -287,9 +287,18 @@ def make_roofline(timings, steps, ms_per_step, peak_gbs, peak_src, clocks, sm_co
                           "thread_instructions_per_cell": round(32.0 * ck["warp_instructions"] / w.n_cells, 2),
                           "achieved_Ginstr_s": round(rate / 1e9, 1), "peak_Ginstr_s": round(issue_peak / 1e9, 1),
                           "frac": round(rate / issue_peak, 4)}
+            if ck.get("fp64_pipe_warp_instructions"):
+                # the tight bound of these kernels: DADD / DFMA / DMUL / DSETP share the fp64 pipe, which accepts one
+                # warp instruction per 2 cycles per scheduler (profiles/r02_issue_rate.md)
+                r64 = ck["fp64_pipe_warp_instructions"] / (v["ms_per_launch"] * 1e-3)
+                e["fp64_pipe"] = {"warp_instructions": ck["fp64_pipe_warp_instructions"],
+                                  "thread_instructions_per_cell": round(32.0 * ck["fp64_pipe_warp_instructions"] / w.n_cells, 2),
+                                  "achieved_Ginstr_s": round(r64 / 1e9, 1), "peak_Ginstr_s": round(0.5 * issue_peak / 1e9, 1),
+                                  "frac": round(r64 / (0.5 * issue_peak), 4)}
         r["kernels"][k] = e
-    if "issue" in r["kernels"][dom]:
-        r["issue"] = r["kernels"][dom]["issue"]
+    for key in ("issue", "fp64_pipe"):
+        if key in r["kernels"][dom]:
+            r[key] = r["kernels"][dom][key]
     return r
 
 
