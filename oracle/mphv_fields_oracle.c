@@ -48,7 +48,8 @@
  * explicit coordinates; interpolation exact for linear fields; Langmuir oscillation at w_p from a
  * cold linear current response; and, through orc_coupled_step with the Vlasov sweeps, the Landau
  * damping rate and frequency of the k = 0.5 mode (gamma = -0.1533, w = 1.4156: the roots of the
- * plasma dispersion function, computed in the test from scipy.special.wofz).
+ * plasma dispersion function, computed in the test from scipy.special.wofz), and the dispersion w^2 = w_p^2 + c^2 K^2
+ * of a transverse light wave in the same plasma.
  * PARITY UNPINNED against the authors' code: PAPER.md prints no field value of theirs.
  *
  * Layouts: every field array is [3][nz][ny][nx], component-major, C order (as E, B of mphv_oracle.c).

@@ -12,6 +12,7 @@ fixes, not against the oracle itself:
   F6 charge current = sum_s q_s j_s
   F7 Landau damping of the k = 0.5 mode through the coupled step: gamma and w against the roots of the
      plasma dispersion function
+  F8 a transverse light wave in a plasma through the coupled step: w^2 = w_p^2 + c^2 K^2
 """
 import itertools
 
@@ -340,3 +341,48 @@ def test_F7_landau_damping_through_the_coupled_step(orc, fld):
     w = _landau_root(k)
     assert abs(omega - w.real) < 0.005 * w.real, (omega, w.real)
     assert abs(gamma - w.imag) < 0.03 * abs(w.imag), (gamma, w.imag)
+
+
+# --------------------------------------------------------------------------------------- F8
+def test_F8_light_wave_in_a_plasma_through_the_coupled_step(orc, fld):
+    """Transverse electromagnetic wave in a cold-ish electron plasma (1D2V: x; vx, vy): E_y = A cos(kx), B = 0, no
+    current at t = 0 is the standing wave at its maximum, E_y(t) = A cos(kx) cos(w t) with the textbook dispersion
+    w^2 = w_p^2 + c^2 K^2, K = (2/dx) sin(k dx / 2) the lattice wavenumber (thermal correction ~ k^2 v_th^2 / w^2 =
+    1e-3). Faraday's law, the curl B term, the transverse current j_y and the sweep along vy are all in the loop:
+    with the current's sign flipped w^2 = c^2 K^2 - w_p^2 = 0 and nothing oscillates."""
+    k, c, A, sg = 1.0, 1.0, 0.01, 0.05
+    nx, nv, vmax = 32, 24, 0.3
+    L = 2 * np.pi / k
+    dx = L / nx
+    grid = orc.Grid((nx, 1, 1), (nv, nv, 1), (PER, PER, PER))
+    box = orc.Box((0.0, 0.0, 0.0), (L, 1.0, 1.0), (-vmax, -vmax, -1.0), (vmax, vmax, 1.0))
+    g = fld.FieldGrid.of(grid, box, c2=c * c, inv_eps0=1.0)
+    v = -vmax + (np.arange(nv) + 0.5) * (2 * vmax / nv)
+    gauss = np.exp(-0.5 * (v / sg) ** 2) / (np.sqrt(2 * np.pi) * sg)
+    f = np.ascontiguousarray(np.broadcast_to((gauss[:, None] * gauss[None, :])[None, None, None, None], grid.shape)).copy()
+    sp = fld.Species(f, grid, box, q=-1.0, q_over_m=-1.0)
+    n0 = orc.moments(f, grid, box)[0].mean()
+    wp2 = n0                                                             # q^2 n / (m eps0), q = m = eps0 = 1
+    x = np.arange(nx) * dx                                               # E_y sits at the cell centres in x (R19, y inactive)
+    E, B = np.zeros(g.shape), np.zeros(g.shape)
+    E[1, 0, 0] = A * np.cos(k * (x + 0.5 * dx))
+    dt, steps = 0.05, 400
+    threads = orc.num_threads()
+    orc.set_num_threads(1)
+    amp, j_now = [], None
+    mode = np.cos(k * (x + 0.5 * dx))
+    for _ in range(steps):
+        moms = fld.coupled_step(g, [sp], E, B, dt, j_now)
+        j_now = [m[1] for m in moms]
+        amp.append(2.0 * (E[1, 0, 0] * mode).mean())
+    orc.set_num_threads(threads)
+    amp = np.array(amp)
+    t = dt * (1 + np.arange(steps))
+    assert np.abs(amp).max() < 1.02 * A and np.abs(amp[-80:]).max() > 0.9 * A      # neither growing nor damped
+    zc = [t[i] - amp[i] * dt / (amp[i + 1] - amp[i]) for i in range(steps - 1) if amp[i] * amp[i + 1] < 0]
+    assert len(zc) >= 8
+    omega = np.pi / np.mean(np.diff(zc))
+    K = 2.0 / dx * np.sin(0.5 * k * dx)
+    want = np.sqrt(wp2 + c * c * K * K)
+    assert abs(omega - want) < 0.005 * want, (omega, want)
+    assert abs(np.abs(E[0]).max()) < 1e-3 * A                            # no longitudinal field is driven
