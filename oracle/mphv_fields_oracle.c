@@ -44,9 +44,9 @@
  * Pins (tests/test_oracle_fields.py): the Yee vacuum dispersion relation sin(w dt/2)/(c dt) =
  * sqrt(sum_d sin^2(k_d dx_d/2)/dx_d^2) (a textbook closed form) through exact return of an eigenmode;
  * div B unchanged to round-off; Gauss's law kept when J obeys the discrete continuity equation;
- * energy bounded; brute-force curl on a 3x3x3 lattice from the definitions of R19 written out with
+ * brute-force curl on a 4x3x5 lattice from the definitions of R19 written out with
  * explicit coordinates; interpolation exact for linear fields; Langmuir oscillation at w_p from a
- * cold linear current response; and, through orc_coupled_step with the Vlasov sweeps, the Landau
+ * cold linear current response; and, through coupled_step (oracle/fields.py) with the Vlasov sweeps, the Landau
  * damping rate and frequency of the k = 0.5 mode (gamma = -0.1533, w = 1.4156: the roots of the
  * plasma dispersion function, computed in the test from scipy.special.wofz), and the dispersion w^2 = w_p^2 + c^2 K^2
  * of a transverse light wave in the same plasma.
