@@ -109,11 +109,12 @@ def _rel_err_by_slab(f_gpu, ref, slab_axis=1):
     return worst
 
 
-@pytest.mark.parametrize("index", [2, 3])
+@pytest.mark.parametrize("index", [2, 3, 4])
 def test_whole_grid_all_steps_of_the_config(orc, index):
-    """BASELINE.json configs 2 and 3 as they are written: the config's 10 full split steps on the WHOLE grid, every
-    cell compared with the oracle (1e-12 after the first step, n x 1e-12 after n), mass to 1e-13 every step,
-    moments every step (config 2) or after the last one (config 3), in the launch configuration bench.py times."""
+    """BASELINE.json configs 2, 3 and 4 as they are written: the config's full split steps (10, 10, 5) on the WHOLE
+    grid, every cell compared with the oracle (1e-12 after the first step, n x 1e-12 after n), mass to 1e-13 every
+    step, moments every step (configs 2, 4) or after the last one (config 3), in the launch configuration bench.py
+    times (config 4: 1.07e9 cells, three spatial and three velocity sweeps)."""
     import torch
     from paper_2305_01487_b200 import inputs, mphv
     w = inputs.config(index)
@@ -126,7 +127,7 @@ def test_whole_grid_all_steps_of_the_config(orc, index):
     mom = sim.alloc_moments()
     ref = f0
     del f0
-    every = index == 2
+    every = w.moments_every_step
     for s in range(w.steps):
         orc.step(ref, grid, box, w.q_over_m, E, B, dt)
         if every or s == w.steps - 1:
