@@ -288,13 +288,15 @@ def make_roofline(timings, steps, ms_per_step, peak_gbs, peak_src, clocks, sm_co
                           "achieved_Ginstr_s": round(rate / 1e9, 1), "peak_Ginstr_s": round(issue_peak / 1e9, 1),
                           "frac": round(rate / issue_peak, 4)}
             if ck.get("fp64_pipe_warp_instructions"):
-                # the tight bound of these kernels: DADD / DFMA / DMUL / DSETP share the fp64 pipe, which accepts one
-                # warp instruction per 2 cycles per scheduler (profiles/r02_issue_rate.md)
-                r64 = ck["fp64_pipe_warp_instructions"] / (v["ms_per_launch"] * 1e-3)
-                e["fp64_pipe"] = {"warp_instructions": ck["fp64_pipe_warp_instructions"],
-                                  "thread_instructions_per_cell": round(32.0 * ck["fp64_pipe_warp_instructions"] / w.n_cells, 2),
-                                  "achieved_Ginstr_s": round(r64 / 1e9, 1), "peak_Ginstr_s": round(0.5 * issue_peak / 1e9, 1),
-                                  "frac": round(r64 / (0.5 * issue_peak), 4)}
+                # the tight bound of these kernels: DADD / DMUL / DSETP occupy the fp64 pipe of a scheduler for 2 cycles
+                # per warp instruction, a DFMA whose three operands are live registers (all of them here) for 3
+                # (bench.py --probe-issue, profiles/r02_issue_rate.md)
+                n64, nfma = ck["fp64_pipe_warp_instructions"], ck.get("dfma_warp_instructions", 0)
+                cycles = 2.0 * (n64 - nfma) + 3.0 * nfma                 # pipe cycles summed over all schedulers
+                floor_ms = cycles / (sm_count * 4) / sm_hz * 1e3
+                e["fp64_pipe"] = {"warp_instructions": n64, "dfma_warp_instructions": nfma,
+                                  "thread_instructions_per_cell": round(32.0 * n64 / w.n_cells, 2),
+                                  "pipe_floor_ms": round(floor_ms, 4), "frac": round(floor_ms / v["ms_per_launch"], 4)}
         r["kernels"][k] = e
     for key in ("issue", "fp64_pipe"):
         if key in r["kernels"][dom]:
@@ -571,7 +573,9 @@ def run_probe_issue():
     torch.cuda.set_device(0)
     torch.zeros(1, device="cuda")
     # kind 3 (DSETP + select) is left out: ptxas drops part of its FSELs, so its instruction count is not exact
-    kinds = {0: "DFMA", 1: "DADD", 2: "select64 (2 FSEL)", 4: "IMAD", 5: "FFMA", 6: "mix: DADD DSETP 2xFSEL DFMA"}
+    kinds = {0: "DFMA", 1: "DADD", 2: "select64 (2 FSEL)", 4: "IMAD", 5: "FFMA", 6: "mix: DADD DSETP 2xFSEL DFMA",
+             7: "DFMA, three live operands", 8: "DADD, two live operands",
+             9: "DFMA (three live) + select64 (two live)"}
     with ClockSampler(0, period=0.005) as clk:
         res = {}
         for k, name in kinds.items():

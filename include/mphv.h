@@ -338,7 +338,9 @@ const char *mphv_plasma_last_error(const mphv_plasma *p);
 /* Issue-rate microbenchmark (the denominator of bench.py's "issue" roofline; method in DESIGN.md sec. 7): runs, on
  * every SM of the current device, `warps_per_scheduler` (1..8) warps per SM scheduler, each thread with 4 independent
  * dependency chains of one instruction kind: 0 DFMA, 1 DADD, 2 64-bit select (2 FSEL), 3 DSETP + 64-bit select,
- * 4 IMAD, 5 FFMA, 6 the limiter's mix (DADD, DSETP, 2 FSEL, DFMA). Returns the best of 3 timed runs in *ms_out
+ * 4 IMAD, 5 FFMA, 6 the limiter's mix (DADD, DSETP, 2 FSEL, DFMA), 7 DFMA with three live register operands,
+ * 8 DADD with two live register operands (0 and 1 keep one or two operands loop-invariant), 9 one such DFMA plus
+ * one 64-bit select of two live operands. Returns the best of 3 timed runs in *ms_out
  * (CUDA events) and the warp instructions ONE scheduler issued in the timed loop in *warp_instructions_out: rate per
  * cycle = warp_instructions / (ms x SM clock). Synchronises the device. */
 int mphv_probe_issue_rate(int kind, int warps_per_scheduler, double *ms_out, double *warp_instructions_out);

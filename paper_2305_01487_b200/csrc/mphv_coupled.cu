@@ -437,6 +437,9 @@ int mphv_probe_issue_rate(int kind, int warps_per_scheduler, double *ms_out, dou
         case PROBE_DSETP_SEL64: probe_kernel<PROBE_DSETP_SEL64><<<sms, threads>>>(out, iters, 1.0000001, 1e-9, 3); break;
         case PROBE_IMAD: probe_kernel<PROBE_IMAD><<<sms, threads>>>(out, iters, 1.0000001, 1e-9, 3); break;
         case PROBE_FFMA: probe_kernel<PROBE_FFMA><<<sms, threads>>>(out, iters, 1.0000001, 1e-9, 3); break;
+        case PROBE_DFMA3: probe_kernel<PROBE_DFMA3><<<sms, threads>>>(out, iters, 1.0000001, 1e-9, 3); break;
+        case PROBE_DADD2: probe_kernel<PROBE_DADD2><<<sms, threads>>>(out, iters, 1.0000001, 1e-9, 3); break;
+        case PROBE_DFMA3_SEL: probe_kernel<PROBE_DFMA3_SEL><<<sms, threads>>>(out, iters, 1.0000001, 1e-9, 3); break;
         default: probe_kernel<PROBE_MIX><<<sms, threads>>>(out, iters, 1.0000001, 1e-9, 3); break;
         }
         cudaEventRecord(e1, 0);
