@@ -314,8 +314,8 @@ const char *mphv_maxwell_last_error(const mphv_maxwell *m);
  *        J' = sum_s q_s j_s[f_s];  Maxwell(dt/2; J').
  * By default everything is enqueued on the field solver's stream (mphv_maxwell_set_stream). With
  * mphv_plasma_set_concurrent(p, 1) every species runs on a CUDA stream of its own, ordered against the field update
- * by events. Measured on B200 (profiles/r02b_two_species.md) that is SLOWER (6.51 vs 6.32 ms per step for ions
- * 40^3 + electrons 36^3 on 128x64): the spatial-sweep kernel and the V-stage kernel each fill an SM's register file,
+ * by events. Measured on B200 (profiles/r02b_two_species.md) that gains nothing (6.26 - 6.51 vs 6.32 ms per step for
+ * ions 40^3 + electrons 36^3 on 128x64): the spatial-sweep kernel and the V-stage kernel each fill an SM's register file,
  * so two species never share an SM, and two spatial sweeps at once split the L2 their row rings live in. Either way
  * the host never waits inside the loop (velocity RANGE checks are deferred, see mphv_set_fields_deferred). The call
  * returns after the last step has been enqueued (the species' streams joined on the field solver's stream);
