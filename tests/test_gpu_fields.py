@@ -238,3 +238,43 @@ def test_landau_damping_on_the_gpu(torch, mphv):
     omega = np.pi / np.mean(np.diff(tp))
     assert abs(omega - 1.4156) < 0.005 * 1.4156, omega
     assert abs(gamma + 0.1533) < 0.03 * 0.1533, gamma
+
+
+def test_light_wave_in_a_plasma_on_the_gpu(torch, mphv):
+    """GPU twin of the oracle pin F8 (no oracle involved): a transverse wave E_y = A cos kx in a cold-ish electron
+    plasma, 1D2V, through mphv_plasma_step: w^2 = w_p^2 + c^2 K^2, K = (2/dx) sin(k dx/2), neither growing nor damped.
+    Faraday's law, the curl B term, the transverse current j_y and the 2V velocity sweeps (fallback kernels) in the loop."""
+    k, c, A, sg = 1.0, 1.0, 0.01, 0.05
+    nx, nv, vmax = 32, 24, 0.3
+    L = 2 * np.pi / k
+    dx = L / nx
+    v = -vmax + (np.arange(nv) + 0.5) * (2 * vmax / nv)
+    gauss = np.exp(-0.5 * (v / sg) ** 2) / (np.sqrt(2 * np.pi) * sg)
+    f0 = np.ascontiguousarray(np.broadcast_to((gauss[:, None] * gauss[None, :])[None, None, None, None], (1, 1, nx, 1, nv, nv))).copy()
+    sim = mphv.Vlasov((nx, 1, 1), (nv, nv, 1), (PER, PER, PER), (0.0, 0.0, 0.0), (L, 1.0, 1.0), (-vmax, -vmax, 0.0), (vmax, vmax, 1.0), q_over_m=-1.0)
+    f = torch.from_numpy(f0).cuda()
+    sim.bind_f(f)
+    wp2 = float(sim.moments()[0].mean())
+    x = (np.arange(nx) + 0.5) * dx
+    E = np.zeros((3, 1, 1, nx)); E[1, 0, 0] = A * np.cos(k * x)
+    mx = mphv.Maxwell((nx, 1, 1), (PER, PER, PER), (dx, 1.0, 1.0), c2=c * c)
+    Ed, Bd = torch.from_numpy(E).cuda(), torch.zeros((3, 1, 1, nx), dtype=torch.float64, device="cuda")
+    mx.bind(Ed, Bd)
+    pl = mphv.Plasma(mx, [sim], [-1.0])
+    dt, steps = 0.05, 400
+    mode = torch.from_numpy(np.cos(k * x)).cuda()
+    amp = []
+    for _ in range(steps):
+        pl.step(dt, 1)
+        amp.append(2.0 * float((Ed[1, 0, 0] * mode).mean()))
+    pl.sync()
+    amp = np.array(amp)
+    t = dt * (1 + np.arange(steps))
+    assert np.abs(amp).max() < 1.02 * A and np.abs(amp[-80:]).max() > 0.9 * A
+    zc = [t[i] - amp[i] * dt / (amp[i + 1] - amp[i]) for i in range(steps - 1) if amp[i] * amp[i + 1] < 0]
+    assert len(zc) >= 8
+    omega = np.pi / np.mean(np.diff(zc))
+    K = 2.0 / dx * np.sin(0.5 * k * dx)
+    want = np.sqrt(wp2 + c * c * K * K)
+    assert abs(omega - want) < 0.005 * want, (omega, want)
+    assert float(Ed[0].abs().max()) < 1e-3 * A
