@@ -57,7 +57,6 @@ struct mphv_ctx {
     int vs_T, vs_grid, vs_variant, vs_bs; size_t vs_smem;
     int vs3_T, vs3_grid; size_t vs3_smem;            // fourth-generation (warp-specialised) whole-V-stage kernel, plain mode (T = 0: shape not covered)
     int vs2_T, vs2_grid; size_t vs2_smem;            // third-generation whole-V-stage kernel, plain mode (T = 0: shape not covered)
-    unsigned char vs_afirst[16], vs_acnt[16];         // stage-A warp items per warp of vstage_kernel (balance_stage_a)   // second-generation whole-V-stage kernel (T = 0: unsupported)
     int sxy_T, sxy_C; size_t sxy_smem;               // fused S_x + S_y kernel (T = 0: unsupported)
     int cube_T, cube_grid, cube_variant, plane_grid; size_t cube_smem, plane_smem;  // whole-V-stage cube kernel launch shape (T = 0: unsupported)
     int vmode;                                       // 0 plain V sweeps, 1 backsubstitution

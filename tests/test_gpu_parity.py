@@ -473,3 +473,24 @@ def test_electron_species_negative_charge_36cubed(torch_cuda, mphv, orc, vmode):
     n_r, j_r, P_r = orc.moments(p.f_ref, p.grid, p.box)
     scale = np.abs(P_r[0]) + np.abs(P_r[3]) + np.abs(P_r[5]) + np.abs(n_r)
     assert np.max(np.abs(j.cpu().numpy() - j_r) / scale) <= 1e-12
+
+
+@pytest.mark.parametrize("gen", ["2", "3", "4"])
+def test_every_generation_of_the_whole_v_stage_kernel_on_40x40_planes(torch_cuda, mphv, orc, gen, monkeypatch):
+    """vstage_kernel, vstage2_kernel and vstage3_kernel (the default) on the velocity planes of the headline config:
+    the V stage with moments against the oracle's three sweeps, every cell. MPHV_VSTAGE_GEN is read by mphv_create."""
+    monkeypatch.setenv("MPHV_VSTAGE_GEN", gen)
+    torch = torch_cuda
+    w = small_workload((8, 6, 1), (40, 40, 40))
+    p = Pair(torch, mphv, orc, w, fusion=3)
+    mom = p.sim.alloc_moments()
+    l0 = p.sim.launches
+    p.sim.stage_v(p.dt, mom)
+    assert p.sim.launches - l0 == 1, "one fused kernel"
+    for d in range(3):
+        orc.sweep_v(p.f_ref, p.grid, p.box, w.q_over_m, p.E, p.B, d, p.dt)
+    assert max(rel_err(p.gpu(), p.f_ref, ax) for ax in (3, 4, 5)) <= TOL_SWEEP
+    n_r, j_r, P_r = orc.moments(p.f_ref, p.grid, p.box)
+    sc = np.abs(P_r[0]) + np.abs(P_r[3]) + np.abs(P_r[5]) + np.abs(n_r)
+    for a_g, a_r in zip(mom, (n_r, j_r, P_r)):
+        assert np.max(np.abs(a_g.cpu().numpy() - a_r) / sc) <= 1e-12
