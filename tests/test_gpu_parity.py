@@ -475,13 +475,16 @@ def test_electron_species_negative_charge_36cubed(torch_cuda, mphv, orc, vmode):
     assert np.max(np.abs(j.cpu().numpy() - j_r) / scale) <= 1e-12
 
 
+@pytest.mark.parametrize("nvz", [40, 14, 12, 8, 4])
 @pytest.mark.parametrize("gen", ["2", "3", "4"])
-def test_every_generation_of_the_whole_v_stage_kernel_on_40x40_planes(torch_cuda, mphv, orc, gen, monkeypatch):
+def test_every_generation_of_the_whole_v_stage_kernel_on_40x40_planes(torch_cuda, mphv, orc, gen, nvz, monkeypatch):
     """vstage_kernel, vstage2_kernel and vstage3_kernel (the default) on the velocity planes of the headline config:
-    the V stage with moments against the oracle's three sweeps, every cell. MPHV_VSTAGE_GEN is read by mphv_create."""
+    the V stage with moments against the oracle's three sweeps, every cell. MPHV_VSTAGE_GEN is read by mphv_create.
+    nvz = 14 / 12: 7 / 6 plane pairs per cube, either side of where vstage3_kernel starts to finish a cube's moments
+    without a barrier; 4: the shortest cube (first and last pair only). 19 x 8 spatial cells: CTAs with one cube and with two."""
     monkeypatch.setenv("MPHV_VSTAGE_GEN", gen)
     torch = torch_cuda
-    w = small_workload((8, 6, 1), (40, 40, 40))
+    w = small_workload((19 if nvz < 40 else 8, 8, 1), (40, 40, nvz))
     p = Pair(torch, mphv, orc, w, fusion=3)
     mom = p.sim.alloc_moments()
     l0 = p.sim.launches
