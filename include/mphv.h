@@ -170,8 +170,10 @@ int mphv_run_host(mphv_ctx *ctx, double *f_host, int nsteps, double dt,
 /* One step of a COUPLED run with f resident on the device (the way the paper's framework drives a Vlasov
  * model: the field solver hands over E, B, the Vlasov model hands back its moments):
  * copies E_host, B_host ([3][nz][ny][nx] each, ideally pinned) to library-owned device memory,
- * mphv_set_fields, mphv_step_moments(dt), copies n, j, P to n_host [ns], j_host [3 ns], P_host [6 ns] and
- * synchronises the stream. f stays in the bound device buffer. Requires bind_f. */
+ * mphv_set_fields_deferred, mphv_step_moments(dt), copies n, j, P to n_host [ns], j_host [3 ns], P_host [6 ns] and
+ * synchronises the stream ONCE, at the end. f stays in the bound device buffer. Requires bind_f. The velocity RANGE
+ * check is the deferred one: MPHV_ERR_RANGE is returned after the step has run, and f is then lost (see
+ * mphv_set_fields_deferred); the context stays in deferred mode until mphv_set_fields is called. */
 int mphv_step_fields_host(mphv_ctx *ctx, const double *E_host, const double *B_host, double dt,
                           double *n_host, double *j_host, double *P_host);
 

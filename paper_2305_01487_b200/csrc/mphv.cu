@@ -1425,15 +1425,15 @@ int mphv_step_fields_host(mphv_ctx *c, const double *E_host, const double *B_hos
     }
     CUDA_TRY(c, cudaMemcpyAsync(c->fld, E_host, 3 * c->ns * sizeof(double), cudaMemcpyHostToDevice, c->stream));
     CUDA_TRY(c, cudaMemcpyAsync(c->fld + 3 * c->ns, B_host, 3 * c->ns * sizeof(double), cudaMemcpyHostToDevice, c->stream));
-    int st = mphv_set_fields(c, c->fld, c->fld + 3 * c->ns);          // also the Courant bound of the new fields
+    // the Courant bound of the new fields stays on the device: the call's one synchronisation is the one at its end
+    int st = mphv_set_fields_deferred(c, c->fld, c->fld + 3 * c->ns);
     if (st != MPHV_OK) return st;
     double *mn = ws_moments(c), *mj = mn + c->ns, *mP = mn + 4 * c->ns;
     if ((st = step_impl(c, dt, mn, mj, mP)) != MPHV_OK) return st;
     CUDA_TRY(c, cudaMemcpyAsync(n_host, mn, c->ns * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     CUDA_TRY(c, cudaMemcpyAsync(j_host, mj, 3 * c->ns * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     CUDA_TRY(c, cudaMemcpyAsync(P_host, mP, 6 * c->ns * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
-    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
-    return MPHV_OK;
+    return mphv_deferred_status(c);                  // synchronises; MPHV_ERR_RANGE if a velocity sweep had |s| >= 1
 }
 
 int mphv_sum_f(mphv_ctx *c, double *sum_dev)

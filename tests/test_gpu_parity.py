@@ -445,6 +445,11 @@ def test_step_fields_host_coupled_step(torch_cuda, mphv, orc):
     scale = np.abs(P_r[0]) + np.abs(P_r[3]) + np.abs(P_r[5]) + np.abs(n_r)
     for a, b in [(nh.numpy(), n_r), (jh.numpy(), j_r), (Ph.numpy(), P_r)]:
         assert np.max(np.abs(a - b) / scale) <= 1e-12
+    # its RANGE check is the deferred one: fields a thousand times larger are reported when the call returns
+    big = torch.from_numpy(1e3 * p.E).pin_memory()
+    with pytest.raises(mphv.MphvError) as ei:
+        p.sim.step_fields_host(big, Bh, p.dt, nh, jh, Ph)
+    assert ei.value.code == mphv.ERR_RANGE
 
 
 @pytest.mark.parametrize("vmode", [0, 1])
