@@ -251,7 +251,7 @@ int mphv_set_vmode(mphv_ctx *ctx, int mode);
  * dimensions; nx not a multiple of 4 or above 256, nvel not a multiple of 8, |s| >= 1 on a periodic axis).
  * Results agree up to fp64 rounding at every level. (For experiments only: the environment variable MPHV_VSTAGE_GEN = 2 or 3,
  * read by mphv_create, keeps the whole-V-stage kernel of levels 2 and 3 to an older generation, vstage_kernel or
- * vstage2_kernel, where the default is vstage3_kernel.) */
+ * vstage2_kernel (backsubstitution mode: vstage_bs_kernel), where the default is vstage3_kernel / vstage3_bs_kernel.) */
 int mphv_set_fusion(mphv_ctx *ctx, int level);
 
 /* mphv_set_fields without the host round trip, for coupled runs that change the fields every step (P:L109,

@@ -11,6 +11,7 @@
 #include "mphv_sxy.cuh"
 #include "mphv_backsub.cuh"
 #include "mphv_vstage_bs.cuh"
+#include "mphv_vstage3_bs.cuh"
 #include "mphv_maxwell.cuh"
 
 #include <cmath>
@@ -55,7 +56,7 @@ struct mphv_ctx {
     int sm_count;
     int vxy_T, vxy_grid; size_t vxy_smem;     // fused V_vx + V_vy plane kernel launch shape (0 = unsupported)
     int vs_T, vs_grid, vs_variant, vs_bs; size_t vs_smem;
-    int vs3_T, vs3_grid; size_t vs3_smem;            // fourth-generation (warp-specialised) whole-V-stage kernel, plain mode (T = 0: shape not covered)
+    int vs3_T, vs3_grid, vs3_bs; size_t vs3_smem;            // fourth-generation (warp-specialised) whole-V-stage kernel, plain mode (T = 0: shape not covered)
     int vs2_T, vs2_grid; size_t vs2_smem;            // third-generation whole-V-stage kernel, plain mode (T = 0: shape not covered)
     int sxy_T, sxy_C; size_t sxy_smem;               // fused S_x + S_y kernel (T = 0: unsupported)
     int cube_T, cube_grid, cube_variant, plane_grid; size_t cube_smem, plane_smem;  // whole-V-stage cube kernel launch shape (T = 0: unsupported)
@@ -340,6 +341,18 @@ template <bool MOM> void *vstage3_fn(int variant)
     default:      return nullptr;
     }
 }
+// the same roles with the three sweeps in face form (backsubstitution mode, mphv_vstage3_bs.cuh)
+#ifndef MPHV_VS3BS_RB40
+#define MPHV_VS3BS_RB40 144
+#define MPHV_VS3BS_RA40 80
+#endif
+template <bool MOM> void *vstage3_bs_fn(int variant)
+{
+    switch (variant) {
+    case CUBE_40: return (void *)vstage3_bs_kernel<MPHV_VS3_NS40, MOM, 40, 40, 5, 20, 320, 512, MPHV_VS3BS_RB40, MPHV_VS3BS_RA40>;
+    default:      return nullptr;
+    }
+}
 int vstage3_threads(int variant) { return variant == CUBE_40 ? 512 : 0; }
 int vstage3_ns(int variant) { return variant == CUBE_40 ? MPHV_VS3_NS40 : 4; }
 size_t vstage3_smem_bytes(int nvx, int nvy, int nvz, int ns)
@@ -396,7 +409,7 @@ int launch_vcube(mphv_ctx *c, double dt, bool with_vz, double *n, double *j, dou
 // V_vx, V_vy, V_vz (+ moments if n != NULL) in one pass over f, two planes per pipeline iteration
 int launch_vstage(mphv_ctx *c, double dt, double *n, double *j, double *P, bool backsub = false)
 {
-    const bool gen4 = !backsub && c->vs3_T > 0;
+    const bool gen4 = c->vs3_T > 0 && (!backsub || c->vs3_bs);
     const bool gen3 = !backsub && !gen4 && c->vs2_T > 0;
     CubeArgs a;
     std::memset(&a, 0, sizeof a);
@@ -411,7 +424,8 @@ int launch_vstage(mphv_ctx *c, double dt, double *n, double *j, double *P, bool 
     a.g = c->gd;
     Timed tm(c, n ? SLOT_VCUBE_MOM : SLOT_VCUBE, (n ? 56.0 : 48.0) * (double)c->nf, 16.0 * (double)c->nf);
     a.K = backsub ? c->bs_K : nullptr;
-    void *fn = backsub ? (n ? vstage_bs_fn<true>(c->vs_variant) : vstage_bs_fn<false>(c->vs_variant))
+    void *fn = backsub && gen4 ? (n ? vstage3_bs_fn<true>(c->vs_variant) : vstage3_bs_fn<false>(c->vs_variant))
+               : backsub ? (n ? vstage_bs_fn<true>(c->vs_variant) : vstage_bs_fn<false>(c->vs_variant))
                : gen4  ? (n ? vstage3_fn<true>(c->vs_variant) : vstage3_fn<false>(c->vs_variant))
                : gen3  ? (n ? vstage2_fn<true>(c->vs_variant) : vstage2_fn<false>(c->vs_variant))
                        : (n ? vstage_fn<true>(c->vs_variant) : vstage_fn<false>(c->vs_variant));
@@ -1030,6 +1044,9 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
                 long long g3 = (long long)c->sm_count;
                 if (g3 > (long long)c->ns) g3 = (long long)c->ns;
                 c->vs3_T = T3; c->vs3_smem = smem3; c->vs3_grid = (int)g3;
+                c->vs3_bs = vstage3_bs_fn<true>(variant) &&
+                            cudaFuncSetAttribute(vstage3_bs_fn<true>(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem3) == cudaSuccess &&
+                            cudaFuncSetAttribute(vstage3_bs_fn<false>(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem3) == cudaSuccess;
             }
             cudaGetLastError();
         }

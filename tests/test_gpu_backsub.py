@@ -127,3 +127,29 @@ def test_fused_backsub_kernel_is_the_one_that_runs(torch_cuda, mphv, orc):
     n0 = p.sim.launches
     p.sim.stage_v(p.dt, mom)
     assert p.sim.launches - n0 == 4, "three sweep kernels and the moments"
+
+
+@pytest.mark.parametrize("nvz", [40, 12, 4])
+@pytest.mark.parametrize("gen", ["3", "4"])
+def test_backsub_whole_v_stage_kernels_on_40x40_planes(torch_cuda, mphv, orc, gen, nvz, monkeypatch):
+    """The velocity planes of the headline config in backsubstitution mode: vstage3_bs_kernel (warp-specialised, the
+    default there) and vstage_bs_kernel (MPHV_VSTAGE_GEN = 3) against the oracle's three backsubstituted sweeps, every
+    cell, with the moments; long cubes, short cubes (moments finished behind a barrier) and the shortest."""
+    monkeypatch.setenv("MPHV_VSTAGE_GEN", gen)
+    w = small_workload((19 if nvz < 40 else 8, 8, 1), (40, 40, nvz))
+    p = Pair(torch_cuda, mphv, orc, w, fusion=3)
+    p.sim.set_vmode(mphv.V_BACKSUB)
+    mom = p.sim.alloc_moments()
+    dt = 1.4 * p.dt
+    p.sim.stage_v(dt, mom)
+    l0 = p.sim.launches
+    p.sim.stage_v(dt, mom)
+    assert p.sim.launches - l0 == 1, "one fused kernel"
+    for _ in range(2):
+        for d in range(3):
+            orc.sweep_v_backsub(p.f_ref, p.grid, p.box, w.q_over_m, p.E, p.B, d, dt)
+    assert max(rel_err(p.gpu(), p.f_ref, ax) for ax in (3, 4, 5)) <= 2 * TOL_SWEEP
+    n_r, j_r, P_r = orc.moments(p.f_ref, p.grid, p.box)
+    sc = np.abs(P_r[0]) + np.abs(P_r[3]) + np.abs(P_r[5]) + np.abs(n_r)
+    for a_g, a_r in zip(mom, (n_r, j_r, P_r)):
+        assert np.max(np.abs(a_g.cpu().numpy() - a_r) / sc) <= 1e-12
