@@ -19,7 +19,10 @@
 #include <cstdio>
 #include <cstring>
 #include <cstdlib>
+#include <map>
+#include <mutex>
 #include <new>
+#include <utility>
 #include <vector>
 
 using namespace mphv;
@@ -95,6 +98,26 @@ void set_err(mphv_ctx *c, const char *fmt, ...)
     va_start(ap, fmt);
     vsnprintf(dst, 512, fmt, ap);
     va_end(ap);
+}
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize belongs to the KERNEL (per device), not to a context: several
+// contexts share the generic kernel instances (and the fused spatial kernel whatever nx), each with its own
+// shared-memory size, so the limit is only ever raised -- a context created later with a smaller grid must not
+// lower it under the feet of an earlier one.
+template <class F> cudaError_t smem_limit(F fn, size_t bytes)
+{
+    static std::mutex mu;
+    static std::map<std::pair<int, const void *>, size_t> limit;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const void *key = reinterpret_cast<const void *>(fn);
+    std::lock_guard<std::mutex> lock(mu);
+    size_t &cur = limit[std::make_pair(dev, key)];
+    if (bytes <= cur) return cudaSuccess;
+    e = cudaFuncSetAttribute(key, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e == cudaSuccess) cur = bytes;
+    return e;
 }
 
 int cuda_fail(mphv_ctx *c, cudaError_t e, const char *what)
@@ -970,7 +993,7 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
         int max_optin = 0;
         cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
         if (nvx + nvy <= T && smem <= (size_t)max_optin &&
-            cudaFuncSetAttribute(vxy_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess) {
+            smem_limit(vxy_kernel<3>, smem) == cudaSuccess) {
             int per_sm = 0;
             if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, vxy_kernel<3>, T, smem) == cudaSuccess && per_sm > 0) {
                 c->vxy_T = T; c->vxy_smem = smem; c->vxy_grid = per_sm * c->sm_count;
@@ -989,8 +1012,8 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
         int max_optin = 0;
         cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
         if (T <= 512 && nvx + nvy <= T && smem <= (size_t)max_optin &&
-            cudaFuncSetAttribute(cube_fn<true>(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess &&
-            cudaFuncSetAttribute(cube_fn<false>(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess) {
+            smem_limit(cube_fn<true>(variant), smem) == cudaSuccess &&
+            smem_limit(cube_fn<false>(variant), smem) == cudaSuccess) {
             int per_sm = 0;
             if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, cube_fn<true>(variant), T, smem) == cudaSuccess && per_sm > 0) {
                 long long g = (long long)per_sm * c->sm_count;
@@ -999,7 +1022,7 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
                 if (g > (long long)c->ns) g = (long long)c->ns;
                 c->cube_T = T; c->cube_smem = smem; c->cube_grid = (int)g; c->cube_variant = variant;
                 c->plane_grid = 0;
-                if (cudaFuncSetAttribute(plane_fn(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)psmem) == cudaSuccess &&
+                if (smem_limit(plane_fn(variant), psmem) == cudaSuccess &&
                     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, plane_fn(variant), T, psmem) == cudaSuccess && per_sm > 0) {
                     long long pg = (long long)per_sm * c->sm_count;
                     if (pg < gmin) pg = ((gmin + c->sm_count - 1) / c->sm_count) * c->sm_count;
@@ -1020,14 +1043,14 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
         int max_optin = 0, per_sm = 0;
         cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
         if (T <= 512 && smem <= (size_t)max_optin &&
-            cudaFuncSetAttribute(vstage_fn<true>(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess &&
-            cudaFuncSetAttribute(vstage_fn<false>(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess &&
+            smem_limit(vstage_fn<true>(variant), smem) == cudaSuccess &&
+            smem_limit(vstage_fn<false>(variant), smem) == cudaSuccess &&
             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, vstage_fn<true>(variant), T, smem) == cudaSuccess && per_sm > 0) {
             long long g = (long long)per_sm * c->sm_count;
             if (g > (long long)c->ns) g = (long long)c->ns;
             c->vs_T = T; c->vs_smem = smem; c->vs_grid = (int)g; c->vs_variant = variant;
-            c->vs_bs = cudaFuncSetAttribute(vstage_bs_fn<true>(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess &&
-                       cudaFuncSetAttribute(vstage_bs_fn<false>(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess;
+            c->vs_bs = smem_limit(vstage_bs_fn<true>(variant), smem) == cudaSuccess &&
+                       smem_limit(vstage_bs_fn<false>(variant), smem) == cudaSuccess;
         }
         cudaGetLastError();
         c->vs3_T = 0;
@@ -1038,15 +1061,15 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
             const int T3 = vstage3_threads(variant);
             int per3 = 0;
             if (smem3 <= (size_t)max_optin &&
-                cudaFuncSetAttribute(vstage3_fn<true>(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem3) == cudaSuccess &&
-                cudaFuncSetAttribute(vstage3_fn<false>(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem3) == cudaSuccess &&
+                smem_limit(vstage3_fn<true>(variant), smem3) == cudaSuccess &&
+                smem_limit(vstage3_fn<false>(variant), smem3) == cudaSuccess &&
                 cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per3, vstage3_fn<true>(variant), T3, smem3) == cudaSuccess && per3 > 0) {
                 long long g3 = (long long)c->sm_count;
                 if (g3 > (long long)c->ns) g3 = (long long)c->ns;
                 c->vs3_T = T3; c->vs3_smem = smem3; c->vs3_grid = (int)g3;
                 c->vs3_bs = vstage3_bs_fn<true>(variant) &&
-                            cudaFuncSetAttribute(vstage3_bs_fn<true>(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem3) == cudaSuccess &&
-                            cudaFuncSetAttribute(vstage3_bs_fn<false>(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem3) == cudaSuccess;
+                            smem_limit(vstage3_bs_fn<true>(variant), smem3) == cudaSuccess &&
+                            smem_limit(vstage3_bs_fn<false>(variant), smem3) == cudaSuccess;
             }
             cudaGetLastError();
         }
@@ -1056,8 +1079,8 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
             const int T2 = vstage2_threads(variant);
             int per2 = 0;
             if (smem2 <= (size_t)max_optin &&
-                cudaFuncSetAttribute(vstage2_fn<true>(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2) == cudaSuccess &&
-                cudaFuncSetAttribute(vstage2_fn<false>(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2) == cudaSuccess &&
+                smem_limit(vstage2_fn<true>(variant), smem2) == cudaSuccess &&
+                smem_limit(vstage2_fn<false>(variant), smem2) == cudaSuccess &&
                 cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per2, vstage2_fn<true>(variant), T2, smem2) == cudaSuccess && per2 > 0) {
                 long long g2 = (long long)per2 * c->sm_count;
                 if (g2 > (long long)c->ns) g2 = (long long)c->ns;
@@ -1086,7 +1109,7 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
                 if (by == grid->bc[1]) smem = sm;
                 for (int bx = 0; bx < 3 && ok; ++bx)
                     ok = sm <= (size_t)max_optin &&
-                         cudaFuncSetAttribute(sxy_fn(C, bx, by), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) == cudaSuccess;
+                         smem_limit(sxy_fn(C, bx, by), sm) == cudaSuccess;
             }
             if (ok) { c->sxy_T = T; c->sxy_C = C; c->sxy_smem = smem; }
         }

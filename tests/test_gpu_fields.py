@@ -278,3 +278,40 @@ def test_light_wave_in_a_plasma_on_the_gpu(torch, mphv):
     want = np.sqrt(wp2 + c * c * K * K)
     assert abs(omega - want) < 0.005 * want, (omega, want)
     assert float(Ed[0].abs().max()) < 1e-3 * A
+
+
+def test_three_species_on_different_velocity_grids(torch, mphv, orc):
+    """Ions, electrons and a light positive third species, each on its own velocity grid (16^3, 20^3, 12^3), coupled
+    through Maxwell: 2 steps of R22 against the oracle (every cell of every f, the fields)."""
+    from paper_2305_01487_b200 import inputs
+    fld = orc.fields
+    wi, we, fi, fe, E, B, dt = _two_species(orc, 16, 8, 16, 20, 16.0)
+    wp = inputs.variant(inputs.electrons_of(wi, mass_ratio=4.0, temp_ratio=0.5, nv=12, vmax=7.0), q_over_m=4.0, seed_offset=900)
+    fp = 0.1 * inputs.make_f0(wp)
+    dt = min(dt, 0.5 * inputs.cfl_dt(wp, 2 * E, 2 * B))
+    c2 = 64.0
+    g = fld.FieldGrid(wi.nx, wi.bc, tuple(wi.dx(d) if wi.nx[d] > 1 else 1.0 for d in range(3)), c2, 1.0)
+    ws, f0s, q = (wi, we, wp), (fi, fe, fp), [1.0, -1.0, 1.0]
+    sims, fdev = [], []
+    for w, f0 in zip(ws, f0s):
+        s = mphv.Vlasov.from_workload(w)
+        fd = torch.from_numpy(f0).cuda()
+        s.bind_f(fd)
+        sims.append(s); fdev.append(fd)
+    mx = mphv.Maxwell.from_workload(wi, c2, 1.0)
+    Ed, Bd = torch.from_numpy(E).cuda(), torch.from_numpy(B).cuda()
+    mx.bind(Ed, Bd)
+    pl = mphv.Plasma(mx, sims, q)
+    species = [fld.Species(f0.copy(), orc.Grid(w.nx, w.nv, w.bc), orc.Box(w.xlo, w.xhi, w.vlo, w.vhi), qq, w.q_over_m)
+               for w, f0, qq in zip(ws, f0s, q)]
+    Er, Br = E.copy(), B.copy()
+    j_now = None
+    for _ in range(2):
+        moms = fld.coupled_step(g, species, Er, Br, dt, j_now)
+        j_now = [m[1] for m in moms]
+    pl.step(dt, 2)
+    pl.sync()
+    for s, sp in enumerate(species):
+        assert max(rel_err(fdev[s].cpu().numpy(), sp.f, ax) for ax in (3, 4, 5)) <= 2 * TOL_SWEEP, s
+    fscale = max(np.abs(Er).max(), np.abs(Br).max()) * max(1.0, c2 * dt / min(g.dx[:2]))
+    assert np.abs(Ed.cpu().numpy() - Er).max() <= 2e-12 * fscale and np.abs(Bd.cpu().numpy() - Br).max() <= 2e-12 * fscale

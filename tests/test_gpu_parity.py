@@ -502,3 +502,16 @@ def test_every_generation_of_the_whole_v_stage_kernel_on_40x40_planes(torch_cuda
     sc = np.abs(P_r[0]) + np.abs(P_r[3]) + np.abs(P_r[5]) + np.abs(n_r)
     for a_g, a_r in zip(mom, (n_r, j_r, P_r)):
         assert np.max(np.abs(a_g.cpu().numpy() - a_r) / sc) <= 1e-12
+
+
+def test_a_later_smaller_context_does_not_break_an_earlier_one(torch_cuda, mphv, orc):
+    """Contexts share the generic kernel instances, whose dynamic shared-memory limit is a property of the KERNEL:
+    creating a second context on a smaller velocity grid must not lower it for the first (regression: the launch of
+    the first context's fused V stage failed with 'invalid argument' once a smaller grid had been created)."""
+    big = Pair(torch_cuda, mphv, orc, small_workload((8, 4, 1), (24, 20, 12)), fusion=3)
+    small = Pair(torch_cuda, mphv, orc, small_workload((8, 4, 1), (12, 12, 8)), fusion=3)
+    for p in (big, small, big):
+        orc.step(p.f_ref, p.grid, p.box, p.w.q_over_m, p.E, p.B, p.dt)
+        p.sim.step(p.dt)
+    assert rel_err(big.gpu(), big.f_ref, AX_V[2]) <= 2 * TOL_SWEEP
+    assert rel_err(small.gpu(), small.f_ref, AX_V[2]) <= TOL_SWEEP
