@@ -56,3 +56,17 @@ def test_committed_counters_match_the_committed_sources():
     import bench
     cj = json.loads((ROOT / "profiles" / "kernel_counters.json").read_text())
     assert cj["csrc_sha16"] == bench.csrc_sha16(), "profiles/kernel_counters.json is stale: re-capture it (DESIGN.md sec. 7)"
+
+
+def test_reference_arm_prints_one_json_line():
+    """bench.py --impl reference: the oracle on the host cores, same metric and workload name, no GPU needed."""
+    import subprocess
+    r = subprocess.run([sys.executable, str(ROOT / "bench.py"), "--impl", "reference", "--steps", "1", "--warmup", "0"],
+                       capture_output=True, text=True, timeout=600, cwd=ROOT)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["metric"] == "phase_space_cell_updates_per_sec" and d["value"] > 0
+    assert d["config"]["workload"] == _W.name and d["cpu_baseline"]["kind"] == "oracle" and d["gpu_launches"] == 0
+    assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["e2e"]["value"] == d["value"]
