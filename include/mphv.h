@@ -181,6 +181,42 @@ int mphv_step_fields_host(mphv_ctx *ctx, const double *E_host, const double *B_h
  * *sum_dev (device, 1 double). Used for the mass checks of BJ (1e-13 relative). */
 int mphv_sum_f(mphv_ctx *ctx, double *sum_dev);
 
+/* The same total for callers that cannot allocate device memory: no context, and no cudaMalloc,
+ * cudaFree or allocating library routine anywhere inside. It is meant for a host code whose own memory
+ * manager already holds all of HBM (a cudaMalloc from inside a library would fail there), and for a
+ * caller inside its time loop, where cudaMalloc / cudaFree would synchronise the device and stall the
+ * other streams. (mphv_create, and therefore mphv_sum_f, gets its workspace from cudaMalloc.)
+ *
+ *   x_dev   [count] fp64, device memory of the CURRENT device, 8-byte aligned, read only
+ *   sum_dev 1 double, device memory of the current device: receives sum_i x_dev[i] (0 for count = 0)
+ *   stream  a cudaStream_t of the current device (NULL = the default stream); the call enqueues two
+ *           kernels on it and returns, *sum_dev is valid once that stream has drained
+ *   err     optional host buffer [err_cap] for the text of a failure (this call has no context, so
+ *           mphv_last_error does not see it); may be NULL
+ *
+ * The per-block partial sums that mphv_sum_f keeps in its context's workspace live here in a static
+ * __device__ array of MPHV_SUM_NOALLOC_MAX_COUNT / MPHV_SUM_NOALLOC_CHUNK = 16384 doubles (128 KiB),
+ * part of the library image: every GPU on which the library is used holds it until the process exits.
+ * Block b sums the fixed chunk x[b*CHUNK, (b+1)*CHUNK), so the result depends on (x, count) only, is
+ * the same bits on every call, and differs from mphv_sum_f's (another summation order) by rounding:
+ * both are Kahan-compensated, |difference| <~ 1e-15 sum|x|.
+ *  - count > MPHV_SUM_NOALLOC_MAX_COUNT (2^30 doubles = 8 GiB of f): MPHV_ERR_RANGE, nothing launched.
+ *    Sum a larger array in pieces, or use mphv_sum_f.
+ *  - The FIRST call on each device looks up the array's device address (cudaGetSymbolAddress, which may
+ *    load the library's kernels on that device) and caches it; make that call during set-up, before any
+ *    stream capture begins. Later calls only launch.
+ *  - All calls on one device share the one array. Nothing in it has to start at zero (each call
+ *    overwrites the entries it reads; what a previous call left beyond them is never read), but two
+ *    calls that may run on the GPU at the same time -- different streams without an ordering between
+ *    them, or several host threads -- race on it and return garbage: order them (same stream, or an
+ *    event). Calls on different devices do not interfere.
+ *  - Errors: MPHV_ERR_ARG (NULL or misaligned pointer), MPHV_ERR_RANGE (above), MPHV_ERR_ARCH (the
+ *    current device is not sm_100), MPHV_ERR_CUDA; outputs untouched on any of them. */
+#define MPHV_SUM_NOALLOC_CHUNK 65536
+#define MPHV_SUM_NOALLOC_MAX_COUNT ((size_t)1 << 30)
+int mphv_sum_noalloc(const double *x_dev, size_t count, double *sum_dev, void *stream,
+                     char *err, size_t err_cap);
+
 /* Number of kernel launches enqueued through this context since creation (for the
  * bench's gpu_launches figure). */
 uint64_t mphv_launch_count(const mphv_ctx *ctx);

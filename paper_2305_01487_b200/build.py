@@ -15,7 +15,7 @@ PKG = Path(__file__).resolve().parent
 ROOT = PKG.parent
 CSRC = PKG / "csrc"
 SO = PKG / "libmphv.so"
-SOURCES = [CSRC / "mphv.cu", CSRC / "mphv_coupled.cu"]
+SOURCES = [CSRC / "mphv.cu", CSRC / "mphv_coupled.cu", CSRC / "mphv_noalloc.cu"]
 DEPS = SOURCES + sorted(CSRC.glob("*.cuh")) + [ROOT / "include" / "mphv.h"]
 
 NVCC_FLAGS = [

@@ -24,7 +24,7 @@ OK, ERR_ARG, ERR_STATE, ERR_RANGE, ERR_CUDA, ERR_ARCH = 0, 1, 2, 3, 4, 5
 SYMBOLS = (
     "mphv_create", "mphv_destroy", "mphv_set_stream", "mphv_f_count", "mphv_space_count",
     "mphv_bind_f", "mphv_set_fields", "mphv_sweep_x", "mphv_sweep_v", "mphv_step",
-    "mphv_moments", "mphv_step_moments", "mphv_run_host", "mphv_step_fields_host", "mphv_sum_f", "mphv_launch_count",
+    "mphv_moments", "mphv_step_moments", "mphv_run_host", "mphv_step_fields_host", "mphv_sum_f", "mphv_sum_noalloc", "mphv_launch_count",
     "mphv_set_fusion", "mphv_set_vmode", "mphv_maxwellian", "mphv_exchange_maxwellian", "mphv_match_moments", "mphv_strerror", "mphv_last_error",
     "mphv_set_timing", "mphv_timing_slots", "mphv_get_timing", "mphv_get_timing_moved",
     "mphv_stage_x", "mphv_stage_x_halo", "mphv_stage_v", "mphv_halo_count", "mphv_pack_halo", "mphv_sweep_x_halo",
@@ -84,6 +84,7 @@ def lib() -> C.CDLL:
         "mphv_run_host": (i32, [vp, vp, i32, dbl, vp, vp, vp]),
         "mphv_step_fields_host": (i32, [vp, vp, vp, dbl, vp, vp, vp]),
         "mphv_sum_f": (i32, [vp, vp]),
+        "mphv_sum_noalloc": (i32, [vp, C.c_size_t, vp, vp, C.c_char_p, C.c_size_t]),
         "mphv_launch_count": (C.c_uint64, [vp]),
         "mphv_set_fusion": (i32, [vp, i32]),
         "mphv_set_vmode": (i32, [vp, i32]),
@@ -241,6 +242,22 @@ def mphv_step_fields_host(ctx, E_host: int, B_host: int, dt: float, n_host: int,
 
 def mphv_sum_f(ctx, sum_dev: int):
     _check(ctx, lib().mphv_sum_f(ctx, sum_dev))
+
+
+SUM_NOALLOC_CHUNK = 65536
+SUM_NOALLOC_MAX_COUNT = 1 << 30
+
+
+def mphv_sum_noalloc(x_dev: int, count: int, sum_dev: int, stream: int | None = None):
+    """Total of ``count`` doubles at ``x_dev`` into the device double at ``sum_dev``, for callers that
+    cannot allocate device memory (their own memory manager holds all of HBM, or they are inside a time
+    loop where cudaMalloc would stall the device): no context, scratch in a static device array of the
+    library. Limits and rules (first call per device during set-up, calls on one device must not overlap
+    on the GPU, ``count`` <= ``SUM_NOALLOC_MAX_COUNT``) in include/mphv.h."""
+    err = C.create_string_buffer(512)
+    st = lib().mphv_sum_noalloc(x_dev, int(count), sum_dev, stream, err, len(err))
+    if st != OK:
+        raise MphvError(st, f"{mphv_strerror(st)}: {err.value.decode(errors='replace')}")
 
 
 def mphv_launch_count(ctx) -> int:
