@@ -163,7 +163,18 @@ int mphv_step_moments(mphv_ctx *ctx, double dt, double *n_dev, double *j_dev, do
  * the outermost active spatial axis) f is cut into up to 16 slabs along that axis and the copy in, the first step,
  * the last step and the copy out are overlapped slab by slab on three streams (each slab is swept as a block of a
  * spatial decomposition, with the neighbouring slabs' boundary layers as ghost cells): a call then costs about one
- * PCIe transfer of f instead of two. Same result up to fp64 rounding. */
+ * PCIe transfer of f instead of two. Same result up to fp64 rounding.
+ * What the slab path needs and costs: (1) f_host must be PINNED (cudaHostAlloc / cudaHostRegister) for the overlap
+ * to happen; with pageable memory every copy blocks the host and the call costs about what the plain path costs.
+ * (2) It is taken only when |s| < 1 on EVERY active spatial axis (the slabs have no scratch buffer; a whole-cell shift
+ * on a periodic axis takes the plain path, which needs the scratch bound by mphv_bind_f). (3) Device memory, allocated
+ * at the first such call and kept until mphv_destroy: up to 16 slab contexts (O(spatial cells) each), a copy of the
+ * fields, and 4 boundary layers per slab -- K*4/n of f for n cells along the slab axis, i.e. a FULL extra copy of f
+ * when n = 64 and K = 16. If that allocation fails the failure is remembered and this context uses the plain path from
+ * then on. (4) With mphv_set_timing on, the kernels of pipelined steps run in the slab contexts and are NOT recorded in
+ * this context's timing slots (mphv_get_timing then under-counts; bench.py times mphv_step, not this call).
+ * (5) On a context in deferred mode (mphv_set_fields_deferred, mphv_step_fields_host) the plain path is taken and the
+ * call ends with mphv_deferred_status: MPHV_ERR_RANGE if a velocity sweep since the last query had |s| >= 1. */
 int mphv_run_host(mphv_ctx *ctx, double *f_host, int nsteps, double dt,
                   double *n_host, double *j_host, double *P_host);
 
@@ -361,7 +372,15 @@ const char *mphv_maxwell_last_error(const mphv_maxwell *m);
  * returns after the last step has been enqueued (the species' streams joined on the field solver's stream);
  * mphv_plasma_sync waits for it and reports a deferred RANGE error. The species contexts are left on the streams
  * the last call used.
- * The first call computes the moments of the initial f_s itself.
+ * The first call computes the moments of the initial f_s itself; later calls reuse the moments the previous call
+ * ended with for their opening Maxwell half step. If a species' f is changed between two calls by anything but
+ * mphv_plasma_step (mphv_exchange_maxwellian or mphv_match_moments at a model border, a re-bind, a direct sweep),
+ * call mphv_plasma_invalidate_moments first: the next mphv_plasma_step then recomputes every species' moments from
+ * the f it finds (one moments pass per species), instead of using the stale current.
+ * mphv_plasma_destroy: while a plasma object lives, its species read the cell-centred fields from buffers the
+ * plasma owns (bound inside mphv_plasma_step). Destroying it un-binds those fields from every species that still
+ * uses them and ends their deferred mode: such a context must get fields again (mphv_set_fields) before its next
+ * sweep, step or mphv_run_host, which otherwise return MPHV_ERR_STATE. Fields the caller bound since are kept.
  * mphv_plasma_moments: device pointers to the latest moments of species s (n [ns], j [3][ns], P [6][ns], owned by
  * the plasma object, valid after mphv_plasma_sync). */
 typedef struct mphv_plasma mphv_plasma;
@@ -370,6 +389,7 @@ int mphv_plasma_destroy(mphv_plasma *p);
 int mphv_plasma_set_concurrent(mphv_plasma *p, int concurrent);
 int mphv_plasma_step(mphv_plasma *p, double dt, int nsteps);
 int mphv_plasma_sync(mphv_plasma *p);
+int mphv_plasma_invalidate_moments(mphv_plasma *p);
 int mphv_plasma_moments(mphv_plasma *p, int s, double **n_dev, double **j_dev, double **P_dev);
 /* centred fields of the last step (device, [3][ns] each, owned by the plasma object) */
 int mphv_plasma_centred_fields(mphv_plasma *p, double **Ec_dev, double **Bc_dev);

@@ -67,6 +67,7 @@ struct mphv_ctx {
     double *bs_K;                                    // device [ns][12] face-displacement coefficients + [3] maxima
     double bs_dt; bool bs_valid; double bs_smax[3];
     struct HostPipe *pipe;   // slab pipeline of mphv_run_host (lazy)
+    bool pipe_failed;        // building it failed once (out of memory): not tried again, mphv_run_host takes the plain path
     uint64_t launches;
     int fusion;
     int timing;
@@ -779,6 +780,7 @@ void destroy_pipe(mphv_ctx *c)
 bool ensure_pipe(mphv_ctx *c)
 {
     if (c->pipe) return true;
+    if (c->pipe_failed) return false;
     int axis = -1;
     for (int d = 2; d >= 0; --d) if (c->grid.nx[d] > 1) { axis = d; break; }
     if (axis < 0) return false;
@@ -819,7 +821,7 @@ bool ensure_pipe(mphv_ctx *c)
              cudaMalloc(&hp->fld, 6 * c->ns * sizeof(double)) == cudaSuccess &&
              cudaMalloc(&hp->mom, 10 * nsk_max * sizeof(double)) == cudaSuccess;
     }
-    if (!ok) { cudaGetLastError(); destroy_pipe(c); return false; }
+    if (!ok) { cudaGetLastError(); destroy_pipe(c); c->pipe_failed = true; return false; }
     return true;
 }
 
@@ -917,6 +919,10 @@ bool pipe_eligible(mphv_ctx *c, double dt)
     int axis = -1;
     for (int d = 2; d >= 0; --d) if (c->grid.nx[d] > 1) { axis = d; break; }
     if (axis < 0 || !(max_courant_x(c, axis, dt) < 1.0)) return false;      // halo sweeps need |s| < 1
+    // the slabs have no scratch buffer (s->scratch = nullptr): a whole-cell shift (|s| >= 1 on a lower, periodic
+    // axis, which the parent accepts when it has one) must take the plain path
+    for (int d = 0; d < axis; ++d)
+        if (c->grid.nx[d] > 1 && !(max_courant_x(c, d, dt) < 1.0)) return false;
     return ensure_pipe(c);
 }
 
@@ -926,6 +932,18 @@ extern "C" {
 
 // for the other translation unit of the library (mphv_coupled.cu): text of mphv_last_error(NULL)
 void mphv_internal_set_create_error(const char *text) { set_err(nullptr, "%s", text ? text : ""); }
+
+// for mphv_plasma_destroy: a species whose fields still are the plasma's centred-field buffers (bound by
+// mphv_set_fields_deferred inside mphv_plasma_step) loses them before that buffer is freed, so that its next
+// sweep fails with MPHV_ERR_STATE instead of reading freed memory. Fields the caller bound since are left alone.
+void mphv_internal_unbind_fields(mphv_ctx *c, const double *E, const double *B)
+{
+    if (!c || c->E != E || c->B != B) return;
+    c->E = c->B = nullptr;
+    c->deferred = false;
+    c->bs_valid = false;
+    for (int d = 0; d < 3; ++d) c->amax[d] = 0.0;
+}
 
 mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_m)
 {
@@ -1448,6 +1466,7 @@ int mphv_run_host(mphv_ctx *c, double *f_host, int nsteps, double dt, double *n_
     if (n_host) CUDA_TRY(c, cudaMemcpyAsync(n_host, mn, c->ns * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     if (j_host) CUDA_TRY(c, cudaMemcpyAsync(j_host, mj, 3 * c->ns * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     if (P_host) CUDA_TRY(c, cudaMemcpyAsync(P_host, mP, 6 * c->ns * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    if (c->deferred) return mphv_deferred_status(c);      // synchronises; a context left in deferred mode reports its RANGE flag here
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     return MPHV_OK;
 }

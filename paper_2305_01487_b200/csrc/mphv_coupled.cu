@@ -40,6 +40,7 @@ struct mphv_plasma {
 
 // defined in mphv.cu (same library): the text buffer mphv_last_error(NULL) returns
 extern "C" void mphv_internal_set_create_error(const char *text);
+extern "C" void mphv_internal_unbind_fields(mphv_ctx *c, const double *E, const double *B);
 
 namespace {
 
@@ -300,6 +301,7 @@ int mphv_plasma_destroy(mphv_plasma *p)
     cudaDeviceSynchronize();
     for (int s = 0; s < p->ns_species; ++s) {
         if (p->sp[s]) mphv_set_stream(p->sp[s], p->m->stream);      // the species leave our streams before these die
+        if (p->sp[s] && p->buf) mphv_internal_unbind_fields(p->sp[s], buf_Ec(p), buf_Bc(p));   // ... and our field buffers
         if (p->sstream[s]) cudaStreamDestroy(p->sstream[s]);
         if (p->ev_mom[s]) cudaEventDestroy(p->ev_mom[s]);
     }
@@ -307,6 +309,13 @@ int mphv_plasma_destroy(mphv_plasma *p)
     if (p->buf) cudaFree(p->buf);
     cudaGetLastError();
     delete p;
+    return MPHV_OK;
+}
+
+int mphv_plasma_invalidate_moments(mphv_plasma *p)
+{
+    if (!p) return MPHV_ERR_ARG;
+    p->have_moments = false;            // the next mphv_plasma_step starts with a moments pass over every species
     return MPHV_OK;
 }
 

@@ -31,7 +31,7 @@ SYMBOLS = (
     "mphv_set_fields_deferred", "mphv_deferred_status",
     "mphv_maxwell_create", "mphv_maxwell_destroy", "mphv_maxwell_set_stream", "mphv_maxwell_bind", "mphv_maxwell_faraday",
     "mphv_maxwell_ampere", "mphv_maxwell_step", "mphv_maxwell_centre", "mphv_maxwell_current", "mphv_maxwell_last_error",
-    "mphv_plasma_create", "mphv_plasma_destroy", "mphv_plasma_set_concurrent", "mphv_plasma_step", "mphv_plasma_sync",
+    "mphv_plasma_create", "mphv_plasma_destroy", "mphv_plasma_set_concurrent", "mphv_plasma_step", "mphv_plasma_sync", "mphv_plasma_invalidate_moments",
     "mphv_plasma_moments", "mphv_plasma_centred_fields", "mphv_plasma_last_error", "mphv_probe_issue_rate",
 )
 
@@ -121,6 +121,7 @@ def lib() -> C.CDLL:
         "mphv_plasma_set_concurrent": (i32, [vp, i32]),
         "mphv_plasma_step": (i32, [vp, dbl, i32]),
         "mphv_plasma_sync": (i32, [vp]),
+        "mphv_plasma_invalidate_moments": (i32, [vp]),
         "mphv_plasma_moments": (i32, [vp, i32, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]),
         "mphv_plasma_centred_fields": (i32, [vp, C.POINTER(vp), C.POINTER(vp)]),
         "mphv_plasma_last_error": (C.c_char_p, [vp]),
@@ -403,6 +404,10 @@ def mphv_plasma_step(p, dt: float, nsteps: int = 1):
 
 def mphv_plasma_sync(p):
     _check_p(p, lib().mphv_plasma_sync(p))
+
+
+def mphv_plasma_invalidate_moments(p):
+    _check_p(p, lib().mphv_plasma_invalidate_moments(p))
 
 
 def mphv_plasma_moments(p, s: int):
@@ -717,6 +722,10 @@ class Plasma:
 
     def sync(self):
         mphv_plasma_sync(self.p)
+
+    def invalidate_moments(self):
+        """Call after changing a species' f by anything but step(): the next step() recomputes the moments."""
+        mphv_plasma_invalidate_moments(self.p)
 
     def moments(self, s: int):
         """(n, j, P) of species s as torch views of the plasma object's device buffers (call sync() first)."""

@@ -186,6 +186,11 @@ def test_deferred_range_check_reports_at_the_next_query(torch, mphv, orc):
         sim.deferred_status()
     assert ei.value.code == mphv.ERR_RANGE
     sim.deferred_status()                                          # the flag was cleared by the query
+    sim.step(dt)                                                   # flag raised again, context still deferred ...
+    fh = torch.from_numpy(f0.copy()).pin_memory()
+    with pytest.raises(mphv.MphvError) as ei:                      # ... and mphv_run_host reports it when it ends
+        sim.run_host(fh, 1, dt)
+    assert ei.value.code == mphv.ERR_RANGE
     sim.set_fields(big, Bd)                                        # back to the immediate check
     with pytest.raises(mphv.MphvError) as ei:
         sim.step(dt)
@@ -315,3 +320,79 @@ def test_three_species_on_different_velocity_grids(torch, mphv, orc):
         assert max(rel_err(fdev[s].cpu().numpy(), sp.f, ax) for ax in (3, 4, 5)) <= 2 * TOL_SWEEP, s
     fscale = max(np.abs(Er).max(), np.abs(Br).max()) * max(1.0, c2 * dt / min(g.dx[:2]))
     assert np.abs(Ed.cpu().numpy() - Er).max() <= 2e-12 * fscale and np.abs(Bd.cpu().numpy() - Br).max() <= 2e-12 * fscale
+
+
+def _small_plasma(torch, mphv, orc, c2=64.0):
+    fld = orc.fields
+    wi, we, fi, fe, E, B, dt = _two_species(orc, 16, 8, 16, 20, 16.0)
+    sims, fdev = [], []
+    for w, f0 in ((wi, fi), (we, fe)):
+        s = mphv.Vlasov.from_workload(w)
+        fd = torch.from_numpy(f0).cuda()
+        s.bind_f(fd)
+        sims.append(s); fdev.append(fd)
+    mx = mphv.Maxwell.from_workload(wi, c2, 1.0)
+    Ed, Bd = torch.from_numpy(E).cuda(), torch.from_numpy(B).cuda()
+    mx.bind(Ed, Bd)
+    return sims, fdev, mx, Ed, Bd, dt, (wi, we, fi, fe, E, B)
+
+
+def test_destroying_the_plasma_unbinds_its_field_buffers_from_the_species(torch, mphv, orc):
+    """After mphv_plasma_destroy a species must not read the freed centred-field buffers: its next step fails with
+    MPHV_ERR_STATE until fields are bound again; fields the caller bound in between are kept."""
+    sims, fdev, mx, Ed, Bd, dt, (wi, we, fi, fe, E, B) = _small_plasma(torch, mphv, orc)
+    pl = mphv.Plasma(mx, sims, [1.0, -1.0])
+    pl.step(dt, 1)
+    pl.sync()
+    own = (torch.from_numpy(E).cuda(), torch.from_numpy(B).cuda())
+    sims[1].set_fields(*own)                       # the caller's own fields on the electrons: must survive
+    pl.close()
+    with pytest.raises(mphv.MphvError) as ei:
+        sims[0].step(dt)
+    assert ei.value.code == mphv.ERR_STATE
+    sims[1].step(dt)                               # still bound, not deferred
+    sims[0].set_fields(*own)
+    sims[0].step(dt)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(fdev[0]).all()) and bool(torch.isfinite(fdev[1]).all())
+
+
+def test_invalidate_moments_after_f_was_changed_between_calls(torch, mphv, orc):
+    """A species' f replaced between two mphv_plasma_step calls: with mphv_plasma_invalidate_moments the second call
+    equals the oracle's coupled step started from the new f (current recomputed), bitwise equal to a fresh plasma
+    object on the same state; without it the stale current of the old f goes into the opening Maxwell half step."""
+    fld = orc.fields
+    c2 = 64.0
+    runs = {}
+    for mode in ("invalidate", "fresh", "stale"):
+        sims, fdev, mx, Ed, Bd, dt, (wi, we, fi, fe, E, B) = _small_plasma(torch, mphv, orc, c2)
+        pl = mphv.Plasma(mx, sims, [1.0, -1.0])
+        pl.step(dt, 1)
+        pl.sync()
+        if mode == "invalidate":                   # the state the reference run below starts from
+            f_mid = [fd.cpu().numpy().copy() for fd in fdev]
+            E_mid, B_mid = Ed.cpu().numpy().copy(), Bd.cpu().numpy().copy()
+        fdev[1].mul_(0.5)                          # e.g. a model-border operation that changed the electrons
+        torch.cuda.synchronize()
+        if mode == "invalidate":
+            pl.invalidate_moments()
+        elif mode == "fresh":
+            pl.close()
+            pl = mphv.Plasma(mx, sims, [1.0, -1.0])
+        pl.step(dt, 1)
+        pl.sync()
+        runs[mode] = [fd.cpu().numpy().copy() for fd in fdev] + [Ed.cpu().numpy().copy(), Bd.cpu().numpy().copy()]
+        pl.close()
+    for a, b in zip(runs["invalidate"], runs["fresh"]):
+        assert np.array_equal(a, b)
+    assert not np.array_equal(runs["invalidate"][2], runs["stale"][2]), "the stale current must have been visible in E"
+    g = fld.FieldGrid(wi.nx, wi.bc, tuple(wi.dx(d) if wi.nx[d] > 1 else 1.0 for d in range(3)), c2, 1.0)
+    f_mid[1] *= 0.5
+    species = [fld.Species(f0, orc.Grid(w.nx, w.nv, w.bc), orc.Box(w.xlo, w.xhi, w.vlo, w.vhi), qq, w.q_over_m)
+               for w, f0, qq in zip((wi, we), f_mid, (1.0, -1.0))]
+    fld.coupled_step(g, species, E_mid, B_mid, dt, None)
+    for s, sp in enumerate(species):
+        assert max(rel_err(runs["invalidate"][s], sp.f, ax) for ax in (3, 4, 5)) <= 2 * TOL_SWEEP, s
+    fscale = max(np.abs(E_mid).max(), np.abs(B_mid).max()) * max(1.0, c2 * dt / min(g.dx[:2]))
+    assert np.abs(runs["invalidate"][2] - E_mid).max() <= 2e-12 * fscale
+    assert np.abs(runs["invalidate"][3] - B_mid).max() <= 2e-12 * fscale

@@ -9,14 +9,15 @@ from parity_util import TOL_SWEEP, moments_err, rel_err
 pytestmark = pytest.mark.gpu
 
 
-def _run(orc, w, nsteps):
+def _run(orc, w, nsteps, dt_scale=1.0, with_scratch=False):
     import torch
     from paper_2305_01487_b200 import inputs, mphv
     f0, E, B, dt = inputs.make_all(w)
+    dt *= dt_scale
     assert f0.nbytes >= 16 << 20, "below the pipeline's size threshold: the test would not test it"
     sim = mphv.Vlasov.from_workload(w)
     f = torch.empty(w.shape, dtype=torch.float64, device="cuda")
-    sim.bind_f(f)
+    sim.bind_f(f, torch.empty_like(f) if with_scratch else None)
     sim.set_fields(torch.from_numpy(E).cuda(), torch.from_numpy(B).cuda())
     fh = torch.from_numpy(f0.copy()).pin_memory()
     nh = torch.empty(w.space_shape, dtype=torch.float64).pin_memory()
@@ -62,3 +63,16 @@ def test_run_host_ragged_slabs(orc):
     """ny = 22 over 5 slabs: slabs of 4 and 5 rows."""
     from paper_2305_01487_b200 import inputs
     _run(orc, inputs.harris2d(32, 22, 16, name="runhost2d_ragged"), 1)
+
+
+def test_run_host_whole_cell_shift_on_a_lower_periodic_axis(orc):
+    """|s| >= 1 along periodic x (the parent context has a scratch buffer, so mphv_step accepts it) on a grid above
+    the pipeline's size threshold: the slabs have no scratch of their own, so this call must take the plain path
+    (it used to run the whole-cell shift of a slab through a NULL scratch pointer)."""
+    from paper_2305_01487_b200 import inputs
+    w = inputs.harris2d(256, 12, 16, name="runhost2d_shift")
+    _, E, B, dt = inputs.make_all(w)
+    scale = 2.5
+    assert np.abs(w.v_centres(0)).max() * dt * scale / w.dx(0) >= 1.0, "the test needs a whole-cell shift along x"
+    assert np.abs(w.v_centres(1)).max() * dt * scale / w.dx(1) < 1.0
+    _run(orc, w, 2, dt_scale=scale, with_scratch=True)
