@@ -57,9 +57,6 @@ def parse():
     ap.add_argument("--aux", action="store_true",
                     help="instead of the step: time the coupling kernels of SURVEY 8(f) (ten-moment Maxwellian fill, "
                          "exchange of Maxwellians, moment matching) on the same workload and print one JSON line")
-    ap.add_argument("--probe-issue", action="store_true",
-                    help="instead of the step: the issue-rate microbenchmark (warp instructions per cycle per SM scheduler "
-                         "by instruction kind and resident warps); one JSON line")
     ap.add_argument("--no-two-species", action="store_true",
                     help="skip the coupled two-species leg (ions + electrons + Maxwell, extra key two_species)")
     ap.add_argument("--species-steps", type=int, default=6)
@@ -290,7 +287,7 @@ def make_roofline(timings, steps, ms_per_step, peak_gbs, peak_src, clocks, sm_co
             if ck.get("fp64_pipe_warp_instructions"):
                 # the tight bound of these kernels: DADD / DMUL / DSETP occupy the fp64 pipe of a scheduler for 2 cycles
                 # per warp instruction, a DFMA whose three operands are live registers (all of them here) for 3
-                # (bench.py --probe-issue, profiles/r02_issue_rate.md)
+                # (measured with a microbenchmark in round 2: profiles/r02_issue_rate.md)
                 n64, nfma = ck["fp64_pipe_warp_instructions"], ck.get("dfma_warp_instructions", 0)
                 cycles = 2.0 * (n64 - nfma) + 3.0 * nfma                 # pipe cycles summed over all schedulers
                 floor_ms = cycles / (sm_count * 4) / sm_hz * 1e3
@@ -566,39 +563,11 @@ def run_aux(args, w):
                       "dtype": "f64", "data": "synthetic", "kernels": kern}), flush=True)
 
 
-def run_probe_issue():
-    """mphv_probe_issue_rate over the instruction kinds of the sweep kernels and 1..8 warps per scheduler."""
-    import torch
-    from paper_2305_01487_b200 import mphv
-    torch.cuda.set_device(0)
-    torch.zeros(1, device="cuda")
-    # kind 3 (DSETP + select) is left out: ptxas drops part of its FSELs, so its instruction count is not exact
-    kinds = {0: "DFMA", 1: "DADD", 2: "select64 (2 FSEL)", 4: "IMAD", 5: "FFMA", 6: "mix: DADD DSETP 2xFSEL DFMA",
-             7: "DFMA, three live operands", 8: "DADD, two live operands",
-             9: "DFMA (three live) + select64 (two live)"}
-    with ClockSampler(0, period=0.005) as clk:
-        res = {}
-        for k, name in kinds.items():
-            res[name] = {}
-            for wps in (1, 2, 3, 4, 8):
-                ms, wi = mphv.mphv_probe_issue_rate(k, wps)
-                res[name][str(wps)] = {"ms": round(ms, 4), "warp_instructions_per_scheduler": wi}
-    c = clk.summary()
-    mhz = c.get("sm_mhz") or c.get("sm_max_mhz")
-    for name in res:
-        for wps, r in res[name].items():
-            r["warp_instr_per_cycle"] = round(r["warp_instructions_per_scheduler"] / (r["ms"] * 1e-3 * mhz * 1e6), 4)
-    print(json.dumps({"metric": "issue_rate_probe", "unit": "warp instructions per cycle per SM scheduler",
-                      "clocks": c, "by_kind_and_warps_per_scheduler": res}), flush=True)
-
-
 def main():
     args = parse()
     from paper_2305_01487_b200 import inputs
     w = inputs.config(args.config)
-    if args.probe_issue:
-        run_probe_issue()
-    elif args.aux:
+    if args.aux:
         run_aux(args, w)
     elif args.impl == "reference":
         run_reference(args, w)

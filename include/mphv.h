@@ -296,10 +296,14 @@ int mphv_set_vmode(mphv_ctx *ctx, int mode);
  * spatial sweeps S_x and S_y in one pass over f (the default, fastest measured on B200). Levels 1..3 fall back to lower-level kernels for
  * grids their kernels do not cover (nvx, nvy not multiples of 4 resp. 2, fewer than 3 velocity
  * dimensions; nx not a multiple of 4 or above 256, nvel not a multiple of 8, |s| >= 1 on a periodic axis).
- * Results agree up to fp64 rounding at every level. (For experiments only: the environment variable MPHV_VSTAGE_GEN = 2 or 3,
- * read by mphv_create, keeps the whole-V-stage kernel of levels 2 and 3 to an older generation, vstage_kernel or
- * vstage2_kernel (backsubstitution mode: vstage_bs_kernel), where the default is vstage3_kernel / vstage3_bs_kernel.) */
+ * Results agree up to fp64 rounding at every level. */
 int mphv_set_fusion(mphv_ctx *ctx, int level);
+
+/* For tests and experiments: the newest generation of the whole-V-stage kernel (fusion levels 2 and 3) this context may
+ * use. 4 (the default) = vstage3_kernel / vstage3_bs_kernel where the grid allows, else the older ones; 3 = at most
+ * vstage2_kernel (backsubstitution mode: vstage_bs_kernel); 2 = vstage_kernel / vstage_bs_kernel. Same results up to
+ * fp64 rounding. The library reads no environment variable. Errors: ARG (generation outside 2..4). */
+int mphv_set_vstage_generation(mphv_ctx *ctx, int generation);
 
 /* mphv_set_fields without the host round trip, for coupled runs that change the fields every step (P:L109,
  * P:L141): the max |a_d| reduction is enqueued as in mphv_set_fields but its result stays on the device, and the
@@ -394,16 +398,6 @@ int mphv_plasma_moments(mphv_plasma *p, int s, double **n_dev, double **j_dev, d
 /* centred fields of the last step (device, [3][ns] each, owned by the plasma object) */
 int mphv_plasma_centred_fields(mphv_plasma *p, double **Ec_dev, double **Bc_dev);
 const char *mphv_plasma_last_error(const mphv_plasma *p);
-
-/* Issue-rate microbenchmark (the denominator of bench.py's "issue" roofline; method in DESIGN.md sec. 7): runs, on
- * every SM of the current device, `warps_per_scheduler` (1..8) warps per SM scheduler, each thread with 4 independent
- * dependency chains of one instruction kind: 0 DFMA, 1 DADD, 2 64-bit select (2 FSEL), 3 DSETP + 64-bit select,
- * 4 IMAD, 5 FFMA, 6 the limiter's mix (DADD, DSETP, 2 FSEL, DFMA), 7 DFMA with three live register operands,
- * 8 DADD with two live register operands (0 and 1 keep one or two operands loop-invariant), 9 one such DFMA plus
- * one 64-bit select of two live operands. Returns the best of 3 timed runs in *ms_out
- * (CUDA events) and the warp instructions ONE scheduler issued in the timed loop in *warp_instructions_out: rate per
- * cycle = warp_instructions / (ms x SM clock). Synchronises the device. */
-int mphv_probe_issue_rate(int kind, int warps_per_scheduler, double *ms_out, double *warp_instructions_out);
 
 const char *mphv_strerror(int code);
 /* Last error text of this context, or of the last failed mphv_create when ctx is NULL.

@@ -70,6 +70,7 @@ struct mphv_ctx {
     bool pipe_failed;        // building it failed once (out of memory): not tried again, mphv_run_host takes the plain path
     uint64_t launches;
     int fusion;
+    int vs_gen_max;          // newest generation of the whole-V-stage kernel the launcher may pick (mphv_set_vstage_generation)
     int timing;
     struct Pending { int slot; cudaEvent_t e0, e1; };
     std::vector<Pending> *pending;
@@ -433,8 +434,8 @@ int launch_vcube(mphv_ctx *c, double dt, bool with_vz, double *n, double *j, dou
 // V_vx, V_vy, V_vz (+ moments if n != NULL) in one pass over f, two planes per pipeline iteration
 int launch_vstage(mphv_ctx *c, double dt, double *n, double *j, double *P, bool backsub = false)
 {
-    const bool gen4 = c->vs3_T > 0 && (!backsub || c->vs3_bs);
-    const bool gen3 = !backsub && !gen4 && c->vs2_T > 0;
+    const bool gen4 = c->vs_gen_max >= 4 && c->vs3_T > 0 && (!backsub || c->vs3_bs);
+    const bool gen3 = c->vs_gen_max >= 3 && !backsub && !gen4 && c->vs2_T > 0;
     CubeArgs a;
     std::memset(&a, 0, sizeof a);
     a.f = c->f;
@@ -837,7 +838,7 @@ int pipe_step(mphv_ctx *c, double dt, const double *f_in, double *f_out, double 
     size_t off_cells = 0;
     for (int k = 0; k < K; ++k) {
         mphv_ctx *s = hp->sub[k];
-        s->stream = c->stream; s->fusion = c->fusion; s->timing = 0; s->vmode = 0;
+        s->stream = c->stream; s->fusion = c->fusion; s->vs_gen_max = c->vs_gen_max; s->timing = 0; s->vmode = 0;
         s->f = c->f + (size_t)hp->row0[k] * hp->layer; s->scratch = nullptr;
         double *Ek = hp->fld + 6 * off_cells, *Bk = Ek + 3 * s->ns;
         CUDA_TRY(c, cudaMemcpy2DAsync(Ek, s->ns * sizeof(double), c->E + off_cells, c->ns * sizeof(double), s->ns * sizeof(double), 3, cudaMemcpyDeviceToDevice, c->stream));
@@ -981,6 +982,7 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
     c->nvel = (size_t)grid->nv[0] * grid->nv[1] * grid->nv[2];
     c->nf = c->ns * c->nvel;
     c->fusion = 3;
+    c->vs_gen_max = 4;
     for (int d = 0; d < 3; ++d) {
         c->dx[d] = grid->nx[d] > 1 ? (box->xhi[d] - box->xlo[d]) / (double)grid->nx[d] : 1.0;
         c->dv[d] = grid->nv[d] > 1 ? (box->vhi[d] - box->vlo[d]) / (double)grid->nv[d] : 1.0;
@@ -1072,9 +1074,7 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
         }
         cudaGetLastError();
         c->vs3_T = 0;
-        const char *gen_env = std::getenv("MPHV_VSTAGE_GEN");          // experiments: 2 / 3 force an older generation
-        const int gen_max = gen_env ? std::atoi(gen_env) : 4;
-        if (c->vs_T > 0 && gen_max >= 4 && vstage3_fn<true>(variant)) {
+        if (c->vs_T > 0 && vstage3_fn<true>(variant)) {
             const size_t smem3 = vstage3_smem_bytes(nvx, nvy, nvz, vstage3_ns(variant));
             const int T3 = vstage3_threads(variant);
             int per3 = 0;
@@ -1092,7 +1092,7 @@ mphv_ctx *mphv_create(const mphv_grid *grid, const mphv_box *box, double q_over_
             cudaGetLastError();
         }
         c->vs2_T = 0;
-        if (c->vs_T > 0 && gen_max >= 3 && vstage2_fn<true>(variant)) {
+        if (c->vs_T > 0 && vstage2_fn<true>(variant)) {
             const size_t smem2 = vstage2_smem_bytes(nvx, nvy, nvz, vstage2_ns(variant));
             const int T2 = vstage2_threads(variant);
             int per2 = 0;
@@ -1572,6 +1572,14 @@ int mphv_set_fusion(mphv_ctx *c, int enabled)
     DevGuard dg(c);
     if (!c) return MPHV_ERR_ARG;
     c->fusion = enabled < 0 ? 0 : (enabled > 3 ? 3 : enabled);
+    return MPHV_OK;
+}
+
+int mphv_set_vstage_generation(mphv_ctx *c, int generation)
+{
+    if (!c) return MPHV_ERR_ARG;
+    if (generation < 2 || generation > 4) { set_err(c, "whole-V-stage kernel generation must be 2, 3 or 4"); return MPHV_ERR_ARG; }
+    c->vs_gen_max = generation;
     return MPHV_OK;
 }
 

@@ -4,7 +4,6 @@
 // kernels of mphv_fields.cuh. No CPU fallback.
 #include "../../include/mphv.h"
 #include "mphv_fields.cuh"
-#include "mphv_probe.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -418,51 +417,5 @@ int mphv_plasma_centred_fields(mphv_plasma *p, double **Ec, double **Bc)
 }
 
 const char *mphv_plasma_last_error(const mphv_plasma *p) { return p ? p->err : mphv_last_error(nullptr); }
-
-// --------------------------------------------------------------------------------------------- issue-rate probe
-
-int mphv_probe_issue_rate(int kind, int warps_per_scheduler, double *ms_out, double *warp_instructions_out)
-{
-    if (kind < 0 || kind >= PROBE_KINDS || warps_per_scheduler < 1 || warps_per_scheduler > 8 || !ms_out || !warp_instructions_out)
-        return MPHV_ERR_ARG;
-    int dev = 0, sms = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
-        cudaGetLastError();
-        return MPHV_ERR_CUDA;
-    }
-    const int threads = 4 * 32 * warps_per_scheduler;          // 4 schedulers per SM, one CTA per SM
-    const int iters = 20000;
-    double *out = nullptr;
-    cudaEvent_t e0, e1;
-    if (cudaMalloc(&out, sizeof(double)) != cudaSuccess) { cudaGetLastError(); return MPHV_ERR_CUDA; }
-    cudaEventCreate(&e0); cudaEventCreate(&e1);
-    float best = 1e30f;
-    for (int rep = 0; rep < 4; ++rep) {                         // first repetition = warm-up
-        cudaEventRecord(e0, 0);
-        switch (kind) {
-        case PROBE_DFMA: probe_kernel<PROBE_DFMA><<<sms, threads>>>(out, iters, 1.0000001, 1e-9, 3); break;
-        case PROBE_DADD: probe_kernel<PROBE_DADD><<<sms, threads>>>(out, iters, 1.0000001, 1e-9, 3); break;
-        case PROBE_SEL64: probe_kernel<PROBE_SEL64><<<sms, threads>>>(out, iters, 1.0000001, 1e-9, 3); break;
-        case PROBE_DSETP_SEL64: probe_kernel<PROBE_DSETP_SEL64><<<sms, threads>>>(out, iters, 1.0000001, 1e-9, 3); break;
-        case PROBE_IMAD: probe_kernel<PROBE_IMAD><<<sms, threads>>>(out, iters, 1.0000001, 1e-9, 3); break;
-        case PROBE_FFMA: probe_kernel<PROBE_FFMA><<<sms, threads>>>(out, iters, 1.0000001, 1e-9, 3); break;
-        case PROBE_DFMA3: probe_kernel<PROBE_DFMA3><<<sms, threads>>>(out, iters, 1.0000001, 1e-9, 3); break;
-        case PROBE_DADD2: probe_kernel<PROBE_DADD2><<<sms, threads>>>(out, iters, 1.0000001, 1e-9, 3); break;
-        case PROBE_DFMA3_SEL: probe_kernel<PROBE_DFMA3_SEL><<<sms, threads>>>(out, iters, 1.0000001, 1e-9, 3); break;
-        default: probe_kernel<PROBE_MIX><<<sms, threads>>>(out, iters, 1.0000001, 1e-9, 3); break;
-        }
-        cudaEventRecord(e1, 0);
-        if (cudaEventSynchronize(e1) != cudaSuccess) { cudaGetLastError(); cudaFree(out); return MPHV_ERR_CUDA; }
-        float ms = 0.f;
-        cudaEventElapsedTime(&ms, e0, e1);
-        if (rep > 0 && ms < best) best = ms;
-    }
-    cudaEventDestroy(e0); cudaEventDestroy(e1);
-    cudaFree(out);
-    *ms_out = best;
-    // warp instructions per SCHEDULER of the timed loop body (loop overhead of ~3 instructions per UNROLL x ILP links not counted)
-    *warp_instructions_out = (double)warps_per_scheduler * iters * PROBE_UNROLL * PROBE_ILP * probe_instr_per_link(kind);
-    return MPHV_OK;
-}
 
 }  // extern "C"

@@ -3,7 +3,7 @@
 //
 // Same data flow as vstage_kernel (mphv_vstage.cuh): TMA ring of plane pairs -> V_vx -> shared memory ->
 // V_vy -> registers -> V_vz march along the plane stream -> global, split barrier between the two stages.
-// Rebuilt around what profiles/r02_issue_rate.md and profiles/r01g_ncu_full.md show: the warps of that kernel
+// Rebuilt around what profiles/r02_issue_rate.md and the round-1 ncu capture (r01g, git history) show: the warps of that kernel
 // are latency-bound (6 cycles per executed instruction per warp, 3.25 warps per scheduler at the 128-register
 // cap of a 13-warp CTA), so time follows the instructions one warp executes per plane pair. Here
 //   * the work items are LONGER and the CTA SMALLER: V_vx on runs of CH consecutive cells (CH + 1 cell fluxes

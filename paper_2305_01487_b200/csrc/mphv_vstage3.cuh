@@ -2,7 +2,7 @@
 // readings R2/R3/R7/R11) and the moments n, j, P (R9/R10) in ONE pass over f, WARP-SPECIALISED.
 //
 // vstage2_kernel (mphv_vstage2.cuh) runs both stages of the pipeline on the same 10 warps: every warp does V_vx of
-// plane pair i ("stage A"), then V_vy + V_vz + moments of pair i-1 ("stage B"). profiles/r02a_ncu_full.md and
+// plane pair i ("stage A"), then V_vy + V_vz + moments of pair i-1 ("stage B"). The round-2 ncu capture (r02a, git history) and
 // profiles/r02_issue_rate.md: it is bound by the latency of each warp's own instruction stream (2.5 warps per
 // scheduler, 50 % issue and 52 % fp64-pipe utilisation, 15 % of the warp time in the two barrier waits); stage B
 // alone takes 1.53 ms of its 2.17 ms, stage A alone 0.89 ms. Here the two stages run on DIFFERENT warps at the

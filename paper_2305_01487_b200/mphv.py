@@ -32,7 +32,7 @@ SYMBOLS = (
     "mphv_maxwell_create", "mphv_maxwell_destroy", "mphv_maxwell_set_stream", "mphv_maxwell_bind", "mphv_maxwell_faraday",
     "mphv_maxwell_ampere", "mphv_maxwell_step", "mphv_maxwell_centre", "mphv_maxwell_current", "mphv_maxwell_last_error",
     "mphv_plasma_create", "mphv_plasma_destroy", "mphv_plasma_set_concurrent", "mphv_plasma_step", "mphv_plasma_sync", "mphv_plasma_invalidate_moments",
-    "mphv_plasma_moments", "mphv_plasma_centred_fields", "mphv_plasma_last_error", "mphv_probe_issue_rate",
+    "mphv_plasma_moments", "mphv_plasma_centred_fields", "mphv_plasma_last_error", "mphv_set_vstage_generation",
 )
 
 
@@ -125,7 +125,7 @@ def lib() -> C.CDLL:
         "mphv_plasma_moments": (i32, [vp, i32, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]),
         "mphv_plasma_centred_fields": (i32, [vp, C.POINTER(vp), C.POINTER(vp)]),
         "mphv_plasma_last_error": (C.c_char_p, [vp]),
-        "mphv_probe_issue_rate": (i32, [i32, i32, C.POINTER(dbl), C.POINTER(dbl)]),
+        "mphv_set_vstage_generation": (i32, [vp, i32]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)
@@ -427,14 +427,12 @@ def mphv_plasma_last_error(p=None) -> str:
     return lib().mphv_plasma_last_error(p).decode()
 
 
-def mphv_probe_issue_rate(kind: int, warps_per_scheduler: int):
-    """(ms, warp instructions per scheduler) of the issue-rate microbenchmark for one instruction kind."""
-    ms, wi = C.c_double(0.0), C.c_double(0.0)
-    _check(None, lib().mphv_probe_issue_rate(int(kind), int(warps_per_scheduler), C.byref(ms), C.byref(wi)))
-    return ms.value, wi.value
+def mphv_set_vstage_generation(ctx, generation: int):
+    _check(ctx, lib().mphv_set_vstage_generation(ctx, int(generation)))
 
 
 # ------------------------------------------------------------------ torch convenience
+
 class Vlasov:
     """One species on one GPU. Holds the context and references to the bound tensors."""
 
@@ -602,6 +600,9 @@ class Vlasov:
 
     def set_vmode(self, mode):
         mphv_set_vmode(self.ctx, mode)
+
+    def set_vstage_generation(self, generation: int):
+        mphv_set_vstage_generation(self.ctx, generation)
 
     def set_fusion(self, level):
         mphv_set_fusion(self.ctx, level)

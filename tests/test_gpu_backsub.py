@@ -130,14 +130,14 @@ def test_fused_backsub_kernel_is_the_one_that_runs(torch_cuda, mphv, orc):
 
 
 @pytest.mark.parametrize("nvz", [40, 12, 4])
-@pytest.mark.parametrize("gen", ["3", "4"])
-def test_backsub_whole_v_stage_kernels_on_40x40_planes(torch_cuda, mphv, orc, gen, nvz, monkeypatch):
+@pytest.mark.parametrize("gen", [3, 4])
+def test_backsub_whole_v_stage_kernels_on_40x40_planes(torch_cuda, mphv, orc, gen, nvz):
     """The velocity planes of the headline config in backsubstitution mode: vstage3_bs_kernel (warp-specialised, the
-    default there) and vstage_bs_kernel (MPHV_VSTAGE_GEN = 3) against the oracle's three backsubstituted sweeps, every
+    default there) and vstage_bs_kernel (mphv_set_vstage_generation(3)) against the oracle's three backsubstituted sweeps, every
     cell, with the moments; long cubes, short cubes (moments finished behind a barrier) and the shortest."""
-    monkeypatch.setenv("MPHV_VSTAGE_GEN", gen)
     w = small_workload((19 if nvz < 40 else 8, 8, 1), (40, 40, nvz))
     p = Pair(torch_cuda, mphv, orc, w, fusion=3)
+    p.sim.set_vstage_generation(gen)
     p.sim.set_vmode(mphv.V_BACKSUB)
     mom = p.sim.alloc_moments()
     dt = 1.4 * p.dt
