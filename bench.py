@@ -325,7 +325,9 @@ def run_mphv(args, w):
         from paper_2305_01487_b200 import halo
         wg = inputs.variant(w, name=f"{w.name}_x{world}", nx=(w.nx[0] * world, w.nx[1], w.nx[2]),
                             xhi=(w.xlo[0] + (w.xhi[0] - w.xlo[0]) * world, w.xhi[1], w.xhi[2]))
-        dec = halo.Decomp(wg.nx, wg.bc, (world, 1, 1))
+        dims = halo.choose_dims(wg.nx, world) if world > 1 else (1, 1, 1)    # x only: the fused X stage (mphv_stage_x_halo)
+        assert dims == (world, 1, 1), dims
+        dec = halo.Decomp(wg.nx, wg.bc, dims)
         Eg, Bg = inputs.make_fields(wg)
         dt = inputs.cfl_dt(wg, Eg, Bg)                       # same on every rank (global fields)
         sl = dec.local_slices(rank)

@@ -94,8 +94,14 @@ class Decomp:
 
 
 def choose_dims(nx: Sequence[int], world: int) -> Tuple[int, int, int]:
-    """Splits `world` ranks over the slowest active spatial axis first (its halo slabs are contiguous
-    in f), then the next one, keeping at least 4 cells per block."""
+    """Process grid for `world` ranks. Preferred: blocks along x ONLY when every block keeps a whole number of
+    4-cell groups and at least 8 cells (nx[0] % (4 world) == 0, nx[0] / world >= 8): that is the decomposition
+    whose X stage runs as one fused pass per step (mphv_stage_x_halo: one exchange, then S_x with ghost cells and
+    S_y in one kernel), and the one bench.py times. Otherwise the ranks go over the slowest active spatial axis
+    first (its halo slabs are contiguous in f), then the next one, keeping at least 4 cells per block; those
+    decompositions take the per-sweep path (pack, exchange, mphv_sweep_x_halo per decomposed axis)."""
+    if world > 1 and nx[0] > 1 and nx[0] % (4 * world) == 0 and nx[0] // world >= 8:
+        return (world, 1, 1)
     dims = [1, 1, 1]
     left = world
     for d in (2, 1, 0):

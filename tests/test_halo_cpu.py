@@ -34,12 +34,20 @@ def test_decomp_bookkeeping():
         halo.Decomp(nx=(6, 8, 1), bc=(0, 1, 0), dims=(2, 1, 1))        # 3-cell blocks
 
 
-def test_choose_dims_prefers_slowest_axis():
-    assert halo.choose_dims((128, 64, 1), 2) == (1, 2, 1)
-    assert halo.choose_dims((128, 64, 1), 8) == (1, 8, 1)
-    assert halo.choose_dims((128, 8, 1), 8) == (4, 2, 1)
-    assert halo.choose_dims((32, 32, 32), 8) == (1, 1, 8)
+def test_choose_dims_prefers_x_only_then_the_slowest_axis():
+    # x only wherever the fused X stage can take it: blocks of whole 4-cell groups, at least 8 cells
+    assert halo.choose_dims((128, 64, 1), 2) == (2, 1, 1)
+    assert halo.choose_dims((128, 64, 1), 8) == (8, 1, 1)
+    assert halo.choose_dims((32, 32, 32), 4) == (4, 1, 1)
+    assert halo.choose_dims((64, 8, 1), 8) == (8, 1, 1)
     assert halo.choose_dims((64, 1, 1), 4) == (4, 1, 1)
+    for n in (1, 2, 4, 8):                                  # bench.py --gpus n: config 3 repeated n times along x
+        assert halo.choose_dims((128 * n, 64, 1), n) == (n, 1, 1)
+    # otherwise the slowest active axis first
+    assert halo.choose_dims((12, 10, 1), 2) == (1, 2, 1)     # 6-cell blocks along x are not whole groups
+    assert halo.choose_dims((32, 32, 32), 8) == (1, 1, 8)    # 4-cell blocks along x are too short
+    assert halo.choose_dims((24, 64, 1), 4) == (1, 4, 1)
+    assert halo.choose_dims((12, 8, 1), 4) == (2, 2, 1)
     with pytest.raises(ValueError):
         halo.choose_dims((4, 4, 1), 8)
 
@@ -87,7 +95,7 @@ def _worker(rank, world, port, dims, kind, q):
     os.environ["MASTER_ADDR"], os.environ["MASTER_PORT"] = "127.0.0.1", str(port)
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
-        w = inputs.harris2d(12, 10, 6) if kind == "2d" else inputs.harris3d(8, 4)
+        w = inputs.harris2d(12, 10, 6) if kind == "2d" else inputs.harris2d(64, 8, 4) if kind == "2dx8" else inputs.harris3d(8, 4)
         dec = halo.Decomp(w.nx, w.bc, dims)
         f0, E, B, dt = inputs.make_all(w)
         dt *= 1.7
@@ -151,4 +159,27 @@ def test_exchange_over_gloo_reproduces_the_global_step(orc, world, dims, kind):
     assert res[0] == "ok", res
     # not bitwise: a block's cell width (xhi - xlo) / n can differ from the global one in the last bit,
     # so its Courant numbers may be one ulp off
+    assert res[1] and res[2] <= 1e-15, f"blocks differ from the global oracle step (max diff / max|f| = {res[2]:.3e})"
+
+
+def test_eight_blocks_along_x_as_bench_gpus_8_decomposes(orc):
+    """world_size 8 over gloo on a 64 x 8 grid with the decomposition choose_dims picks (x only, 8-cell blocks): the
+    bookkeeping of `bench.py --gpus 8` (block offsets, periodic wrap across 8 ranks, both ghost slabs of every block)."""
+    import torch.multiprocessing as mp
+    dims = halo.choose_dims((64, 8, 1), 8)
+    assert dims == (8, 1, 1)
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, 8, port, dims, "2dx8", q)) for r in range(8)]
+    for p in procs:
+        p.start()
+    try:
+        res = q.get(timeout=400)
+    finally:
+        for p in procs:
+            p.join(timeout=90)
+            if p.is_alive():
+                p.kill()
+    assert res[0] == "ok", res
     assert res[1] and res[2] <= 1e-15, f"blocks differ from the global oracle step (max diff / max|f| = {res[2]:.3e})"
