@@ -63,7 +63,8 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
-    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU work of the oracle sample")
+    ap.add_argument("--cpu-seconds", type=float, default=30.0,
+                    help="CPU work the oracle sample is sized for over 20 steps (estimated; about a third of it on a 16-core box)")
     return ap.parse_args()
 
 
@@ -154,22 +155,24 @@ def oracle_sample(w, cpu_seconds: float):
     return sub
 
 
-def time_oracle(w, steps: int, warmup: int, cpu_seconds: float, adapt: bool = False):
-    """Times oracle.step + oracle.moments, as they stand, on a bounded sample of workload w."""
+SAMPLE_STEPS = 20          # the oracle sample is sized for cpu_seconds of work over this many steps (= the default --steps)
+
+
+def time_oracle(w, steps: int, warmup: int, cpu_seconds: float):
+    """Times oracle.step + oracle.moments, as they stand, on a bounded sample of workload w. ONE sample per workload:
+    the cpu_baseline leg and the --impl reference arm time the same sub-block (sized for cpu_seconds / SAMPLE_STEPS of
+    oracle work per step), and with default flags the same number of steps; a long reference run (steps + warmup
+    above 200) shrinks the block so that the whole run stays within a few minutes."""
     import oracle
     from paper_2305_01487_b200 import inputs
-    sub = oracle_sample(w, cpu_seconds / max(1, steps + warmup))
+    sub = oracle_sample(w, min(cpu_seconds / SAMPLE_STEPS, 150.0 / max(1, steps + warmup)))
     f0, E, B, _ = inputs.make_all(sub)
     dt = 0.5 * inputs.cfl_dt(sub, E, B)          # safely inside |s| < 1 on the sub-block
     grid, box = oracle.Grid(sub.nx, sub.nv, sub.bc), oracle.Box(sub.xlo, sub.xhi, sub.vlo, sub.vhi)
     f = f0.copy()
-    tw = time.perf_counter()
     for _ in range(warmup):
         oracle.step(f, grid, box, sub.q_over_m, E, B, dt)
         oracle.moments(f, grid, box)
-    tw = (time.perf_counter() - tw) / max(1, warmup)
-    if adapt and warmup and tw > 0:                              # enough steps for ~cpu_seconds of timed work
-        steps = int(min(16, max(steps, round(cpu_seconds / tw))))
     t0 = time.perf_counter()
     for _ in range(steps):
         oracle.step(f, grid, box, sub.q_over_m, E, B, dt)
@@ -188,7 +191,7 @@ def run_reference(args, w):
     if rank != 0:
         return
     steps, warmup = max(1, args.steps), max(0, args.warmup)
-    r = time_oracle(w, steps, warmup, cpu_seconds=max(10.0, min(120.0, 3.0 * (steps + warmup))))
+    r = time_oracle(w, steps, warmup, args.cpu_seconds)
     line = {
         "impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
         "steps": steps, "warmup": warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True,
@@ -477,7 +480,7 @@ def run_mphv(args, w):
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         del f0
-        line["cpu_baseline"] = {k: v for k, v in time_oracle(w, 2, 1, args.cpu_seconds, adapt=True).items() if k != "ms_per_step"}
+        line["cpu_baseline"] = {k: v for k, v in time_oracle(w, min(SAMPLE_STEPS, max(1, args.steps)), 1, args.cpu_seconds).items() if k != "ms_per_step"}
 
     if rank == 0:
         print(json.dumps(line), flush=True)
